@@ -1,0 +1,127 @@
+/*
+ * fire.h -- C ABI of libfire: batched stochastic cellular-automata fire propagation on a raster
+ * landscape plus the per-simulation fitness reduction against a reference burned map, the hot
+ * path of arXiv 1701.03549 (Denham & Laneri), for NVIDIA B200 (sm_100a).
+ *
+ * The problem as the paper states it: given raster layers for vegetation, slope, aspect and wind
+ * direction (Sec. 3.1), a parameter vector beta of Eq. 1, an
+ * ignition point and a random seed, run the cellular automaton
+ * until the fire stops by itself and score the final burnt map
+ * against a reference map with Eq. 2.  The GA / Monte-Carlo search that calls
+ * this millions of times (App. B, C) stays on the host.
+ *
+ * Conventions (DESIGN.md "Readings of the paper" R-4..R-9)
+ *   - rasters are row-major [H][W]; row 0 is north, x grows east; angles are radians, compass
+ *     bearings clockwise from north.  `aspect` = bearing the slope faces (downslope), `wind` =
+ *     bearing the wind blows TOWARD, `slope` = inclination angle in [0, pi/2).
+ *   - veg: 0 = impossible to burn, 1 = forest (I_f = 1), >= 2 = other burnable fuel (I_f = 0).
+ *   - direction d = 0..7 = N, NE, E, SE, S, SW, W, NW is the direction of travel from the burning
+ *     cell to the target cell; thresholds are indexed [cell of the TARGET][d].
+ *   - bitmaps: cell (x, y) is bit (x & 31) (LSB = lowest x) of 32-bit word y*ceil(W/32) + (x >> 5);
+ *     tail bits of a row are zero.
+ *
+ * Pointers: every array argument is a DEVICE pointer on the handle's device unless its name
+ * ends in `_host`.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ * Ownership: the caller owns every array; the library borrows it until the enqueued work is
+ * done.  The handle owns covariates, thresholds, scratch planes and queues.
+ * Asynchrony: every call only enqueues work on `stream` unless stated otherwise; outputs are valid
+ * once the caller has synchronised the stream.  A handle must not be used from two streams at once.
+ * Errors: 0 on success, a negative FIRE_E* code otherwise.  The library never throws, aborts or
+ * prints.  Faults only the device can see (ignition outside the lattice or on a non-burnable
+ * cell, sim_param outside [0, P)) are not errors: that simulation burns nothing, steps = 0 (R-12).
+ * There is no CPU fallback: without a CUDA device every call returns FIRE_ECUDA.
+ */
+#ifndef FIRE_H
+#define FIRE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FIRE_OK       0
+#define FIRE_EINVAL  (-1)   /* null pointer, non-positive size, R < 2, lattice larger than 8192 x 8192 */
+#define FIRE_ENOMEM  (-2)   /* device allocation failed */
+#define FIRE_ESTATE  (-3)   /* simulate before fire_params_upload, p out of range in download */
+#define FIRE_ECUDA   (-4)   /* a CUDA call failed (sticky), or no CUDA device */
+
+#define FIRE_METRIC_DELTA    0   /* Eq. 2: (#(A u A*) - #(A n A*)) / #A, 0 = perfect overlap */
+#define FIRE_METRIC_JACCARD  1   /* #(A n A*) / #(A u A*) */
+
+typedef struct fire_landscape fire_landscape;   /* opaque; one handle = one device */
+
+/* Landscape ingest.  Derives and keeps, per cell, the
+ * covariates of Eq. 1 in double precision (I_f, psi, omega_d, sigma_d) and the burnable bitmap.
+ * veg u8[H][W]; slope, aspect, wind f32[H][W].  Precondition (R-20): finite values, 0 <= slope < pi/2.
+ * The rasters may be freed once `stream` has passed this point.  1 <= W, H <= 8192. */
+int fire_landscape_create(fire_landscape** out, const uint8_t* veg, const float* slope,
+                          const float* aspect, const float* wind, int32_t W, int32_t H, void* stream);
+
+/* Frees everything the handle owns.  Synchronises the device. */
+int fire_landscape_destroy(fire_landscape* L);
+
+/* Contagion-threshold precompute (a2; Eq. 1).  beta f32[P][5] = (beta_0 .. beta_4).
+ * For every parameter vector p, burnable cell c and direction d:
+ *   T[p][c][d] = min(rint(2^32 / (1 + exp(-(b0 + b1 I_f + b2 psi + b3 omega_d + b4 sigma_d)))), 2^32 - 1)
+ * in IEEE double, no FMA contraction; T = 0 on non-burnable cells.  A trial succeeds iff
+ * rnd < T or T == 2^32 - 1 (R-11).  Replaces any previous table; allocates P*W*H*32 bytes. */
+int fire_params_upload(fire_landscape* L, const float* beta, int32_t P, void* stream);
+
+/* Batch of S independent simulations (a3-a6).
+ * ignitions i32[S][2] = (x, y); sim_param i32[S] in [0, P); seeds u64[S];
+ * sim_ids i32[S] or NULL: the `sim` field of the random-number key (NULL = 0..S-1), so that a
+ * shard of a larger batch reproduces the same fires.  max_steps: 0 = until extinction.
+ * The random word of trial (seed, sim, step t, target cell c = y*W + x, direction d) is word d & 3 of
+ * Philox4x32-10(counter = (c, t, sim, d >> 2), key = (seed & 0xffffffff, seed >> 32)) (R-3).
+ * out_burned u32[S][H][ceil(W/32)] final burnt map (every word is written);
+ * out_steps u32[S] or NULL: number of CA steps until the fire stopped;
+ * out_trials u64[S] or NULL: number of (target cell, direction) Bernoulli trials performed. */
+int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, const int32_t* sim_param,
+                        const uint64_t* seeds, const int32_t* sim_ids, int32_t S, uint32_t max_steps,
+                        uint32_t* out_burned, uint32_t* out_steps, uint64_t* out_trials, void* stream);
+
+/* Fitness reduction (a7; Eq. 2).  reference u32[H][ceil(W/32)] = A, burned
+ * u32[S][H][ceil(W/32)] = A*.  out_counts u32[S][2] or NULL = (I, N*) with I = #(A n A*), N* = #A*;
+ * out_score f32[S]: metric 0 = (float)(N + N* - 2I) / (float)N, metric 1 = (float)I / (float)(N + N* - I),
+ * N = #A; one IEEE divide (N = 0 gives inf/NaN, not an error).  out_ref_area u32[1] or NULL = N. */
+int fire_fitness(fire_landscape* L, const uint32_t* reference, const uint32_t* burned, int32_t S,
+                 int32_t metric, float* out_score, uint32_t* out_counts, uint32_t* out_ref_area, void* stream);
+
+/* Per-candidate statistics over R replicates (a8; BASELINE config 4).
+ * counts u32[G*R][2] = (I, N*), candidate-major; x = ref_area + N* - 2I.
+ * out_sums u64[G][2] = (sum x, sum x^2); out_mean_var f64[G][2] = mean and sample variance (R-16)
+ * of delta = x / ref_area:  mean = sum x / (R N),  var = (R sum x^2 - (sum x)^2) / (R (R-1)) / N^2. */
+int fire_fitness_group_stats(const uint32_t* counts, uint32_t ref_area, int32_t G, int32_t R,
+                             uint64_t* out_sums, double* out_mean_var, void* stream);
+
+/* Test hook: copies the threshold table of parameter vector p to out u32[H][W][8] (device). */
+int fire_thresholds_download(fire_landscape* L, int32_t p, uint32_t* out, void* stream);
+
+/* One GA generation with HOST buffers (end-to-end path): copies beta, ignitions, sim_param, seeds
+ * (and sim_ids if not NULL) and the reference bitmap to the device, runs fire_params_upload,
+ * fire_simulate_batch and fire_fitness on `stream`, copies scores (and counts / steps if not NULL)
+ * back and SYNCHRONISES the stream.  Host arrays should be page-locked for full copy bandwidth.
+ * The burnt maps stay on the device: *out_burned_dev (if not NULL) receives a device pointer to
+ * u32[S][H][ceil(W/32)] owned by the handle, valid until the next call on this handle. */
+int fire_generation_host(fire_landscape* L, const float* beta_host, int32_t P,
+                         const int32_t* ignitions_host, const int32_t* sim_param_host,
+                         const uint64_t* seeds_host, const int32_t* sim_ids_host, int32_t S,
+                         uint32_t max_steps, const uint32_t* reference_host, int32_t metric,
+                         float* out_score_host, uint32_t* out_counts_host, uint32_t* out_steps_host,
+                         uint32_t** out_burned_dev, void* stream);
+
+/* Number of kernel launches the library has enqueued on this handle so far (bench.py's gpu_launches). */
+int64_t fire_launch_count(const fire_landscape* L);
+
+/* Tuning knob (tests use it to show results do not depend on launch geometry, pin P-9):
+ * threads per CTA of the propagation kernel (multiple of 32, 64..1024; 0 = default) and CTAs per SM
+ * (0 = default). */
+int fire_set_launch_geometry(fire_landscape* L, int32_t threads_per_cta, int32_t ctas_per_sm);
+
+const char* fire_error_string(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FIRE_H */
