@@ -114,10 +114,23 @@ int fire_generation_host(fire_landscape* L, const float* beta_host, int32_t P,
 /* Number of kernel launches the library has enqueued on this handle so far (bench.py's gpu_launches). */
 int64_t fire_launch_count(const fire_landscape* L);
 
+/* Device timing of the propagation kernel alone (bench.py's roofline): while enabled, every
+ * fire_simulate_batch brackets its propagation kernel with a pair of CUDA events on `stream` (at most 64
+ * pairs are kept between reads).  fire_profile_read waits for the recorded events, writes their elapsed
+ * milliseconds, oldest first, to ms_host (HOST memory, max_entries floats), sets *n_out and forgets them. */
+int fire_set_profiling(fire_landscape* L, int32_t enabled);
+int fire_profile_read(fire_landscape* L, float* ms_host, int32_t max_entries, int32_t* n_out);
+
 /* Tuning knob (tests use it to show results do not depend on launch geometry, pin P-9):
  * threads per CTA of the propagation kernel (multiple of 32, 64..1024; 0 = default) and CTAs per SM
  * (0 = default). */
 int fire_set_launch_geometry(fire_landscape* L, int32_t threads_per_cta, int32_t ctas_per_sm);
+
+/* Test hook (pin P-9): capacity, in cells, of the per-CTA frontier list of the propagation kernel:
+ * the first `shared_entries` live in shared memory, the rest up to `total_entries` in a global spill
+ * area; a simulation whose burning front ever exceeds `total_entries` is redone by the list-free
+ * rescue kernel.  Results never depend on these values.  0 = default. */
+int fire_set_list_capacity(fire_landscape* L, int32_t shared_entries, int32_t total_entries);
 
 const char* fire_error_string(int code);
 

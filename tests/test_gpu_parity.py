@@ -1,0 +1,324 @@
+"""`-m gpu`: parity of the CUDA path (through the C ABI) with the CPU oracle, element by element.
+
+Layers:
+  1. thresholds: GPU table vs oracle table; > 1 count apart = failure, <= 1-count differences are
+     counted and reported (north_star).
+  2. propagation with the oracle fed the GPU's OWN threshold table: bit-exact, no excuses.
+  3. end to end, each side on its own thresholds: bit-exact burned maps, steps, trials and fitness
+     on all five configs -- configs 3-5 at full size against values stored by
+     oracle/make_workloads.py (oracle only), in the launch configuration bench.py times.
+"""
+import json
+
+import numpy as np
+import pytest
+
+from conftest import GOLDEN, unpack_bitmap
+from paper_1701_03549_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():                       # collected on the CPU box too; never runs there
+    pytest.skip("needs a CUDA device", allow_module_level=True)
+
+import gpu_helpers as gh                                 # noqa: E402
+from paper_1701_03549_b200 import libfire as lf          # noqa: E402
+
+
+def small_landscape(rng, H, W, nonburn=0.2, nveg=4):
+    veg = rng.choice(nveg, size=(H, W), p=[nonburn] + [(1 - nonburn) / (nveg - 1)] * (nveg - 1)).astype(np.uint8)
+    return {"veg": veg, "slope": rng.uniform(0, 0.7, (H, W)).astype(np.float32),
+            "aspect": rng.uniform(0, 2 * np.pi, (H, W)).astype(np.float32),
+            "wind": rng.uniform(0, 2 * np.pi, (H, W)).astype(np.float32), "W": W, "H": H}
+
+
+def orc_landscape(orc, ls):
+    return orc.Landscape(ls["veg"], ls["slope"], ls["aspect"], ls["wind"])
+
+
+def report(request, **kv):
+    line = " ".join(f"{k}={v}" for k, v in kv.items())
+    print(f"\n[parity] {request.node.name}: {line}")
+    request.node.user_properties.append(("parity", line))
+
+
+# ---------------------------------------------------------------------------------- layer 1
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_thresholds_within_one_count(orc, request, cfg):
+    w = wl.load_workload(cfg)
+    Lo = orc_landscape(orc, w.landscape)
+    L = gh.make_landscape(w.landscape)
+    gh.upload(L, np.vstack([w.betas, w.ref_beta[None, :]]))
+    n_diff = n_tot = 0
+    for p in range(w.P + 1):
+        beta = w.betas[p] if p < w.P else w.ref_beta
+        g = gh.thresholds(L, p).astype(np.int64)
+        o = orc.threshold_table(Lo, beta).astype(np.int64)
+        d = np.abs(g - o)
+        assert d.max() <= 1, f"cfg{cfg} p={p}: threshold differs by {d.max()} counts at {np.unravel_index(d.argmax(), d.shape)}"
+        assert ((g == 0) == (o == 0))[w.landscape["veg"] == 0].all()
+        n_diff += int((d != 0).sum()); n_tot += d.size
+    report(request, entries=n_tot, one_count_differences=n_diff, fraction=f"{n_diff / n_tot:.2e}")
+    assert n_diff / n_tot < 1e-3
+    L.close()
+
+
+def test_thresholds_extreme_and_special_values(orc, request):
+    rng = np.random.default_rng(5)
+    ls = small_landscape(rng, 37, 45)
+    ls["slope"][0, :8] = [0.0, np.float32(5 * np.pi / 180), np.nextafter(np.float32(5 * np.pi / 180), np.float32(1)), 1.5, 1e-30, 0.3, 0.3, 0.3]
+    ls["aspect"][0, :8] = [0.0, 0.0, np.float32(7 * np.pi / 4), np.float32(np.pi / 2), 0.0, np.float32(np.pi / 2), np.float32(np.pi), np.float32(2 * np.pi)]
+    ls["wind"][1, :4] = [0.0, np.float32(np.pi / 4), np.float32(np.pi), np.float32(2 * np.pi)]
+    betas = np.array([[0, 0, 0, 0, 0], [-50, 0, 0, 0, 0], [50, 0, 0, 0, 0], [-5, -10, 5, 18.1, -5], [23, 0, 0, 0, 0],
+                      [-23, 0, 0, 0, 0], [30, -30, 30, -30, 30], [-1.5, 0.25, -0.75, 2.5, 1.25]], np.float32)
+    L = gh.make_landscape(ls); Lo = orc_landscape(orc, ls)
+    gh.upload(L, betas)
+    n_diff = 0
+    for p in range(len(betas)):
+        g = gh.thresholds(L, p).astype(np.int64); o = orc.threshold_table(Lo, betas[p]).astype(np.int64)
+        assert np.abs(g - o).max() <= 1, (p, np.abs(g - o).max())
+        n_diff += int((g != o).sum())
+    burn = ls["veg"] != 0
+    assert (gh.thresholds(L, 0)[burn] == 2 ** 31).all()              # beta = 0 -> p = 1/2 exactly
+    assert (gh.thresholds(L, 1) == 0).all()                          # p == 0
+    assert (gh.thresholds(L, 2)[burn] == 0xFFFFFFFF).all()           # p == 1 (certain)
+    assert (gh.thresholds(L, 2)[~burn] == 0).all()
+    report(request, one_count_differences=n_diff)
+    L.close()
+
+
+# ---------------------------------------------------------------------------------- layer 2
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_propagation_bit_exact_on_gpu_thresholds(orc, request, cfg):
+    w = wl.load_workload(cfg)
+    Lo = orc_landscape(orc, w.landscape)
+    L = gh.make_landscape(w.landscape)
+    gh.upload(L, w.betas)
+    g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    tables = [gh.thresholds(L, p) for p in range(w.P)]
+    o = orc.simulate_batch(Lo, w.betas, w.ignitions, w.sim_param, w.seeds, tables=tables)
+    bad = [s for s in range(w.S) if not (g["burned"][s] == o["burned"][s]).all()]
+    assert not bad, f"cfg{cfg}: burned maps differ for sims {bad[:10]}"
+    assert (g["steps"] == o["steps"]).all() and (g["trials"] == o["trials"]).all()
+    report(request, sims=w.S, trials=int(o["trials"].sum()), cells_burned=int(gh.popcount(o["burned"]).sum()))
+    L.close()
+
+
+# ---------------------------------------------------------------------------------- layer 3
+@pytest.mark.parametrize("cfg", [1, 2, 4, 3, 5])
+def test_end_to_end_matches_oracle_golden(request, cfg):
+    """Full-size configs in bench.py's launch configuration vs values stored by oracle/make_workloads.py."""
+    e = json.loads((GOLDEN / f"cfg{cfg}_expected.json").read_text())
+    w = wl.load_workload(cfg)
+    L = gh.make_landscape(w.landscape)
+    gh.upload(L, np.vstack([w.betas, w.ref_beta[None, :]]))      # the reference vector rides along as index P
+    g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds, keep_device=True)
+    assert (g["steps"] == np.array(e["steps"], np.uint32)).all(), np.flatnonzero(g["steps"] != np.array(e["steps"]))[:10]
+    assert (g["trials"] == np.array(e["trials"], np.uint64)).all()
+    # reference fire: its own simulation (sim id 0) from the stored vector, ignition and seed
+    ref = gh.simulate(L, [w.ref_ignition], [w.P], [w.ref_seed], sim_ids=[0])
+    assert gh.digest(ref["burned"][0]) == e["ref_digest"] and int(ref["steps"][0]) == e["ref_steps"]
+    counts, score, N = gh.fitness(L, ref["burned"][0], g["burned"], w.metric)
+    assert N == e["ref_area"]
+    assert (counts[:, 0] == np.array(e["intersection"], np.uint32)).all()
+    assert (counts[:, 1] == np.array(e["area"], np.uint32)).all()
+    # every burned map, bit for bit (digest of the canonical words), in slabs to bound host memory
+    S = w.S
+    slab = max(1, (256 << 20) // (L.H * L.Ww * 4))
+    bad = []
+    for s0 in range(0, S, slab):
+        hb = g["burned"][s0:s0 + slab].cpu().numpy().view(np.uint32)
+        bad += [s0 + i for i in range(hb.shape[0]) if gh.digest(hb[i]) != e["digest"][s0 + i]]
+    assert not bad, f"cfg{cfg}: {len(bad)} burned maps differ, first {bad[:10]}"
+    # scores: one IEEE divide of the exact integers, restated here in numpy float32
+    I = counts[:, 0].astype(np.int64); A = counts[:, 1].astype(np.int64)
+    with np.errstate(all="ignore"):
+        want = ((N + A - 2 * I).astype(np.float32) / np.float32(N)) if w.metric == 0 else \
+               (I.astype(np.float32) / (N + A - I).astype(np.float32))
+    assert np.array_equal(score, want.astype(np.float32), equal_nan=True)
+    if w.groups:
+        G, R = w.groups
+        sums, mv = gh.group_stats(counts, N, G, R)
+        x = (N + A - 2 * I).reshape(G, R)
+        assert (sums[:, 0] == x.sum(1)).all() and (sums[:, 1] == (x * x).sum(1)).all()
+        d = x / N
+        assert np.allclose(mv[:, 0], d.mean(1), rtol=1e-13) and np.allclose(mv[:, 1], d.var(1, ddof=1), rtol=1e-9, atol=1e-18)
+    report(request, sims=S, trials=e["totals"]["trials"], burned_cells=e["totals"]["area"], launches=lf.fire_launch_count(L))
+    L.close()
+
+
+# ---------------------------------------------------------------------------------- edge cases
+def test_limits_p0_p1_and_invalid_sims(orc):
+    rng = np.random.default_rng(21)
+    ls = small_landscape(rng, 50, 77, nonburn=0.4)          # width not a multiple of 32: ragged tail
+    ls["veg"][0, 0] = 1; ls["veg"][49, 76] = 2              # burnable corners: fires that start on the lattice edge
+    Lo = orc_landscape(orc, ls)
+    L = gh.make_landscape(ls)
+    betas = np.array([[-50, 0, 0, 0, 0], [50, 0, 0, 0, 0], [-1, 0, 0.2, 1, 0.5]], np.float32)
+    gh.upload(L, betas)
+    ys, xs = np.nonzero(ls["veg"]); nb_y, nb_x = np.nonzero(ls["veg"] == 0)
+    ign = [[xs[3], ys[3]], [xs[3], ys[3]], [xs[40], ys[40]], [nb_x[0], nb_y[0]], [-1, 5], [77, 5], [5, 50], [5, -1],
+           [xs[9], ys[9]], [xs[9], ys[9]], [0, 0], [76, 49]]
+    par = [0, 1, 2, 1, 1, 1, 1, 1, 3, -1, 1, 1]
+    seeds = np.arange(len(par), dtype=np.uint64) + 77
+    g = gh.simulate(L, ign, par, seeds)
+    o = orc.simulate_batch(Lo, betas, np.array(ign, np.int32), np.array(par, np.int32), seeds)
+    assert (g["burned"] == o["burned"]).all() and (g["steps"] == o["steps"]).all() and (g["trials"] == o["trials"]).all()
+    b = unpack_bitmap(g["burned"], 77)
+    assert b[0].sum() == 1 and g["steps"][0] == 1                                   # p == 0: ignition only
+    from scipy import ndimage
+    lab, _ = ndimage.label(ls["veg"] != 0, structure=np.ones((3, 3)))
+    assert (b[1] == (lab == lab[ys[3], xs[3]])).all()                               # p == 1: the 8-connected component
+    for s in (3, 4, 5, 6, 7, 8, 9):
+        assert b[s].sum() == 0 and g["steps"][s] == 0 and g["trials"][s] == 0       # R-12
+    assert (g["burned"][:, :, -1] >> np.uint32(77 - 64)).max() == 0                  # tail bits stay zero
+    L.close()
+
+
+@pytest.mark.parametrize("H,W", [(1, 1), (1, 200), (130, 1), (3, 33), (64, 64), (97, 161)])
+def test_odd_shapes_bit_exact(orc, H, W):
+    rng = np.random.default_rng(H * 1000 + W)
+    ls = small_landscape(rng, H, W, nonburn=0.1)
+    Lo = orc_landscape(orc, ls); L = gh.make_landscape(ls)
+    betas = np.array([[0.3, -0.5, 0.3, 1.0, 0.5], [-0.6, 0, 0, 0.5, 0], [50, 0, 0, 0, 0]], np.float32)
+    gh.upload(L, betas)
+    S = 24
+    ign = np.stack([rng.integers(0, W, S), rng.integers(0, H, S)], 1).astype(np.int32)
+    par = (np.arange(S) % 3).astype(np.int32); seeds = rng.integers(0, 2 ** 63, S).astype(np.uint64)
+    g = gh.simulate(L, ign, par, seeds)
+    tables = [gh.thresholds(L, p) for p in range(3)]
+    o = orc.simulate_batch(Lo, betas, ign, par, seeds, tables=tables)
+    assert (g["burned"] == o["burned"]).all() and (g["steps"] == o["steps"]).all() and (g["trials"] == o["trials"]).all()
+    L.close()
+
+
+def test_max_steps_and_sim_ids(orc):
+    w = wl.load_workload(1)
+    Lo = orc_landscape(orc, w.landscape); L = gh.make_landscape(w.landscape)
+    gh.upload(L, w.betas)
+    for ms in (1, 2, 7):
+        g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds, max_steps=ms)
+        o = orc.simulate_batch(Lo, w.betas, w.ignitions, w.sim_param, w.seeds, max_steps=ms)
+        assert (g["burned"] == o["burned"]).all() and (g["steps"] == o["steps"]).all()
+    # a shard of the batch with explicit sim ids reproduces the same fires (multi-GPU sharding)
+    full = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    sl = wl.shard_sims(w.S, 1, 3)
+    part = gh.simulate(L, w.ignitions[sl], w.sim_param[sl], w.seeds[sl], sim_ids=np.arange(w.S, dtype=np.int32)[sl])
+    assert (part["burned"] == full["burned"][sl]).all() and (part["trials"] == full["trials"][sl]).all()
+    L.close()
+
+
+def test_results_do_not_depend_on_launch_geometry_or_list_capacity(request):
+    """Pin P-9: same bytes for every CTA size, residency, shared/global list split, and through the rescue kernel."""
+    w = wl.load_workload(2)
+    L = gh.make_landscape(w.landscape)
+    gh.upload(L, w.betas)
+    base = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    again = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    assert (base["burned"] == again["burned"]).all()
+    for threads, per_sm, shared, total in [(32, 1, 0, 0), (64, 8, 0, 0), (128, 2, 0, 0), (512, 1, 0, 0), (1024, 1, 0, 0),
+                                           (256, 4, 16, 0), (256, 4, 5, 4096), (96, 3, 1, 0),
+                                           (256, 4, 8, 8), (128, 4, 64, 100), (256, 2, 0, 1)]:
+        lf.fire_set_launch_geometry(L, threads, per_sm)
+        lf.fire_set_list_capacity(L, shared, total)
+        g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+        ok = (g["burned"] == base["burned"]).all(axis=(1, 2))
+        assert ok.all(), f"geometry {(threads, per_sm, shared, total)}: sims {np.flatnonzero(~ok)[:10]} differ"
+        assert (g["steps"] == base["steps"]).all() and (g["trials"] == base["trials"]).all(), (threads, per_sm, shared, total)
+    L.close()
+
+
+# ---------------------------------------------------------------------------------- fitness
+def test_fitness_counts_and_scores_bit_exact(orc):
+    rng = np.random.default_rng(3)
+    for H, W, S in [(64, 64, 7), (50, 77, 5), (1, 1, 2), (1024, 1024, 3), (33, 4100, 4)]:
+        ls = small_landscape(rng, H, W)
+        L = gh.make_landscape(ls)
+        Ww = (W + 31) // 32
+        mask = np.zeros((Ww * 32,), bool); mask[:W] = True
+        tail = np.packbits(mask, bitorder="little").view("<u4")
+        ref = rng.integers(0, 2 ** 32, (H, Ww), dtype=np.uint32) & tail
+        burned = rng.integers(0, 2 ** 32, (S, H, Ww), dtype=np.uint32) & tail
+        burned[0] = ref; burned[1] = 0
+        if S > 2:
+            burned[2] = ~ref & tail
+        for metric in (0, 1):
+            counts, score, N = gh.fitness(L, ref, burned, metric)
+            oc, os_, oN = orc.fitness(ref, burned, W, metric)
+            assert N == oN and (counts == oc).all()
+            assert np.array_equal(score.view(np.uint32), os_.view(np.uint32))                    # bit-exact floats
+        # empty reference: N = 0 gives inf / NaN, not an error
+        counts, score, N = gh.fitness(L, np.zeros_like(ref), burned, 0)
+        oc, os_, oN = orc.fitness(np.zeros_like(ref), burned, W, 0)
+        assert N == 0 and np.array_equal(score, os_, equal_nan=True)
+        L.close()
+
+
+def test_group_stats_bit_exact(orc):
+    rng = np.random.default_rng(4)
+    for G, R, N in [(1, 2, 10), (1024, 16, 35785), (33, 50, 2 ** 24), (7, 3, 1)]:
+        Ns = rng.integers(0, 2 ** 24, G * R).astype(np.uint32)
+        I = (rng.random(G * R) * np.minimum(Ns, N)).astype(np.uint32)
+        counts = np.stack([I, Ns], 1)
+        sums, mv = gh.group_stats(counts, N, G, R)
+        osums, omv = orc.group_stats(counts, N, G, R)
+        assert (sums == osums).all() and np.array_equal(mv.view(np.uint64), omv.view(np.uint64))
+
+
+def test_generation_host_matches_device_path():
+    w = wl.load_workload(2)
+    L = gh.make_landscape(w.landscape)
+    gh.upload(L, np.vstack([w.betas, w.ref_beta[None, :]]))
+    ref = gh.simulate(L, [w.ref_ignition], [w.P], [w.ref_seed], sim_ids=[0])["burned"][0]
+    gh.upload(L, w.betas)
+    g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds, keep_device=True)
+    counts, score, N = gh.fitness(L, ref, g["burned"], w.metric)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_score = torch.empty(w.S, dtype=torch.float32).pin_memory()
+    h_counts = torch.empty((w.S, 2), dtype=torch.int32).pin_memory()
+    h_steps = torch.empty(w.S, dtype=torch.int32).pin_memory()
+    ptr = lf.fire_generation_host(L, pin(w.betas), pin(w.ignitions), pin(w.sim_param), pin(w.seeds.view(np.int64)),
+                                  pin(ref.view(np.int32)), w.metric, h_score, h_counts, h_steps)
+    assert ptr != 0
+    assert np.array_equal(h_score.numpy().view(np.uint32), score.view(np.uint32))
+    assert (h_counts.numpy().view(np.uint32) == counts).all() and (h_steps.numpy().view(np.uint32) == g["steps"]).all()
+    L.close()
+
+
+def test_errors_are_codes_not_crashes():
+    w = wl.load_workload(1)
+    L = gh.make_landscape(w.landscape)
+    with pytest.raises(lf.FireError) as ei:                                          # simulate before params
+        gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    assert ei.value.code == lf.FIRE_ESTATE
+    gh.upload(L, w.betas)
+    with pytest.raises(lf.FireError) as ei:
+        lf.fire_thresholds_download(L, 99, torch.empty((L.H, L.W, 8), dtype=torch.int32, device="cuda"))
+    assert ei.value.code == lf.FIRE_ESTATE
+    with pytest.raises(lf.FireError) as ei:
+        lf.fire_set_launch_geometry(L, 100, 1)
+    assert ei.value.code == lf.FIRE_EINVAL
+    with pytest.raises(TypeError):
+        lf.fire_params_upload(L, torch.zeros((2, 5)))                                # host tensor: there is no CPU path
+    assert lf.load().fire_landscape_destroy(None) == lf.FIRE_EINVAL
+    L.close()
+
+
+# ---------------------------------------------------------------------------------- distribution (P-8)
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_burned_area_distribution_ks(orc, request, cfg):
+    """GPU seeds 0..999 vs oracle seeds 1000..1999 at the reference (near-transition) vector: KS p > 0.01."""
+    from scipy.stats import ks_2samp
+    w = wl.load_workload(cfg)
+    Lo = orc_landscape(orc, w.landscape); L = gh.make_landscape(w.landscape)
+    gh.upload(L, w.ref_beta[None, :])
+    n = 1000
+    ign = np.tile(np.array([w.ref_ignition], np.int32), (n, 1)); par = np.zeros(n, np.int32)
+    g = gh.simulate(L, ign, par, np.arange(n, dtype=np.uint64))
+    o = orc.simulate_batch(Lo, w.ref_beta[None, :], ign, par, np.arange(n, 2 * n, dtype=np.uint64))
+    ga, oa = gh.popcount(g["burned"]), gh.popcount(o["burned"])
+    ks = ks_2samp(ga, oa)
+    report(request, gpu_mean_area=f"{ga.mean():.1f}", oracle_mean_area=f"{oa.mean():.1f}", ks_p=f"{ks.pvalue:.3f}")
+    assert ks.pvalue > 0.01
+    L.close()
