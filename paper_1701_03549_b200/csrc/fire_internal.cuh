@@ -24,7 +24,8 @@ struct fire_landscape {
     double*   omega;         // [8][cells]  cos(wind - phi_d)
     uint32_t* burnable;      // [H][Ww] bitmap
 
-    // a2: thresholds, [P][cells][8] u32 = one 32 B DRAM sector per (p, target cell)
+    // a2: thresholds, [P][cells][8] u32, SOURCE-indexed: thr[p][b][d] = T(target b + offset(d), direction d);
+    // one 32 B DRAM sector holds the 8 outgoing trials of a burning cell b
     uint32_t* thr;
     size_t    thr_capacity;  // bytes allocated
     int       P;             // 0 until fire_params_upload
@@ -32,6 +33,14 @@ struct fire_landscape {
     size_t    beta_capacity;
 
     // a3-a6: propagation scratch
+    int Tw, Th;                   // 8 x 8-cell tiles per row / column of the lattice: ceil(W/8), ceil(H/8)
+    uint64_t* burnable_tiles;     // [Th][Tw] burnable bitmap in tile layout: bit (y&7)*8 + (x&7) of tile (y>>3, x>>3)
+    uint64_t* tiles;              // [S][Th][Tw] susceptible plane (burnable & ~burned) of every simulation of a batch
+    size_t    tiles_capacity;     // bytes
+    uint32_t* order;              // [S] launch order of the simulations (largest expected first)
+    size_t    order_capacity;     // bytes
+    float*    param_mean;         // [P] mean contagion probability per parameter vector (written by fire_params_upload)
+    size_t    param_mean_capacity;
     unsigned int* work_counter;   // [2] next sim index for the fast kernel / the rescue kernel
     uint32_t* status;             // [S] 0 = finished by the fast kernel, 1 = needs the rescue kernel
     size_t    status_capacity;    // entries

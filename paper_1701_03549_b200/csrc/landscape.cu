@@ -61,9 +61,19 @@ fire_covariates_kernel(const uint8_t* __restrict__ veg, const float* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------ a2
-// One thread per cell, looping over a group of parameter vectors with the cell's covariates held in
-// registers.  For a fixed p a warp writes 32 x 32 B = 1 KiB contiguous (two 16 B stores per thread).
+// The table is SOURCE-indexed: thr[p][b][d] = T of the trial "burning cell b spreads in direction d",
+// i.e. Eq. 1 evaluated with the covariates of the TARGET b + offset(d) ("covariates of the
+// target cell"); 0 where the target is non-burnable.  The 8 outgoing trials of one burning cell are one
+// 32 B DRAM sector, and a cell burns for exactly one step, so the propagation kernel
+// reads every sector it needs exactly once.  Slots whose target lies outside the lattice are never
+// written and never read.
+//
+// One thread per TARGET cell of a 32 x 8 tile, covariates in registers, loop over a group of parameter
+// vectors.  The 8 thresholds of a target go through shared memory to the slots of their 8 sources, so
+// that sources whose targets all lie in the tile (30 x 6 of 32 x 8) are written as whole sectors; the
+// others are completed, 4 B at a time, by the neighbouring tiles (merged in L2).
 #define FIRE_THR_PGROUP 8
+constexpr int kThrTX = 32, kThrTY = 8;
 
 __device__ __forceinline__ uint32_t fire_threshold_from_x(double x)
 {
@@ -73,48 +83,123 @@ __device__ __forceinline__ uint32_t fire_threshold_from_x(double x)
     return (uint32_t)(t > 0xFFFFFFFFll ? 0xFFFFFFFFll : (t < 0 ? 0 : t));
 }
 
-__global__ void __launch_bounds__(128)
-fire_thresholds_kernel(const float* __restrict__ beta, int P, size_t cells,
+// x of Eq. 1 for one (target, direction): every operation one IEEE double operation, in the order of C-3
+__device__ __forceinline__ uint32_t fire_threshold(double b0, double b1, double b2, double b3, double b4,
+                                                   double If, double ps, double om, double sg)
+{
+    const double base = __dadd_rn(__dadd_rn(b0, __dmul_rn(b1, If)), __dmul_rn(b2, ps));
+    const double x = __dadd_rn(__dadd_rn(base, __dmul_rn(b3, om)), __dmul_rn(b4, sg));
+    return fire_threshold_from_x(x);
+}
+
+__global__ void __launch_bounds__(kThrTX * kThrTY)
+fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int tiles_x,
                        const uint8_t* __restrict__ flags, const uint8_t* __restrict__ uphill,
                        const double* __restrict__ psi, const double* __restrict__ tan_slope,
-                       const double* __restrict__ omega, uint32_t* __restrict__ thr)
+                       const double* __restrict__ omega, uint32_t* __restrict__ thr, float* __restrict__ param_mean)
 {
     __shared__ double sb[FIRE_THR_PGROUP][5];
+    __shared__ float s_mean[FIRE_THR_PGROUP];
+    __shared__ uint32_t sT[8][kThrTY + 2][kThrTX + 2];                    // [d][source row + 1][source column + 1]
+    const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
     const int p0 = blockIdx.y * FIRE_THR_PGROUP;
     const int np = min(FIRE_THR_PGROUP, P - p0);
-    if (threadIdx.x < np * 5) sb[threadIdx.x / 5][threadIdx.x % 5] = (double)beta[(size_t)p0 * 5 + threadIdx.x];
-    __syncthreads();
-    const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= cells) return;
-    const uint32_t f = flags[c];
-    uint4* out = reinterpret_cast<uint4*>(thr) + ((size_t)p0 * cells + c) * 2;
-    if ((f & 1u) == 0) {                                                  // impossible to burn: T = 0
-        for (int q = 0; q < np; ++q) {
-            out[0] = make_uint4(0, 0, 0, 0); out[1] = make_uint4(0, 0, 0, 0);
-            out += cells * 2;
-        }
-        return;
-    }
-    const double If = (f & 2u) ? 1.0 : 0.0;
-    const double ps = psi[c], ts = tan_slope[c];
-    const uint32_t up = uphill[c];
-    double om[8];
+    if (tid < np * 5) sb[tid / 5][tid % 5] = (double)beta[(size_t)p0 * 5 + tid];
+    if (tid < FIRE_THR_PGROUP) s_mean[tid] = 0.0f;
+    const int x0 = (int)(blockIdx.x % tiles_x) * kThrTX, y0 = (int)(blockIdx.x / tiles_x) * kThrTY;
+    const int x = x0 + lx, y = y0 + ly;
+    const size_t cells = (size_t)W * H;
+    const bool inside = x < W && y < H;
+    const size_t c = inside ? (size_t)y * W + x : 0;
+    const uint32_t f = inside ? flags[c] : 0u;
+    const bool live = (f & 1u) != 0;                                      // impossible to burn: T = 0
+    double If = 0.0, ps = 0.0, ts = 0.0, om[8];
+    uint32_t up = 0;
 #pragma unroll
-    for (int d = 0; d < 8; ++d) om[d] = omega[(size_t)d * cells + c];
+    for (int d = 0; d < 8; ++d) om[d] = 0.0;
+    if (live) {
+        If = (f & 2u) ? 1.0 : 0.0;
+        ps = psi[c]; ts = tan_slope[c]; up = uphill[c];
+#pragma unroll
+        for (int d = 0; d < 8; ++d) om[d] = omega[(size_t)d * cells + c];
+    }
+    // the sources this thread writes out: its own cell, and (threads 0..83) one cell of the ring around the tile
+    int hx = -2, hy = -2;                                                 // ring cell in tile coordinates, if any
+    if (tid < 2 * kThrTX) { hx = tid & 31; hy = (tid < kThrTX) ? -1 : kThrTY; }
+    else if (tid < 2 * kThrTX + 2 * kThrTY) { const int k = tid - 2 * kThrTX; hx = (k < kThrTY) ? -1 : kThrTX; hy = k % kThrTY; }
+    else if (tid < 2 * kThrTX + 2 * kThrTY + 4) { const int k = tid - 2 * kThrTX - 2 * kThrTY; hx = (k & 1) ? kThrTX : -1; hy = (k & 2) ? kThrTY : -1; }
+    __syncthreads();
     for (int q = 0; q < np; ++q) {
         const double b0 = sb[q][0], b1 = sb[q][1], b2 = sb[q][2], b3 = sb[q][3], b4 = sb[q][4];
-        const double base = __dadd_rn(__dadd_rn(b0, __dmul_rn(b1, If)), __dmul_rn(b2, ps));
-        uint32_t T[8];
+        float fsum = 0.0f;
 #pragma unroll
         for (int d = 0; d < 8; ++d) {
-            const double sg = ((up >> d) & 1u) ? ts : 0.0;
-            const double x = __dadd_rn(__dadd_rn(base, __dmul_rn(b3, om[d])), __dmul_rn(b4, sg));
-            T[d] = fire_threshold_from_x(x);
+            uint32_t T = 0u;
+            if (live) T = fire_threshold(b0, b1, b2, b3, b4, If, ps, om[d], ((up >> d) & 1u) ? ts : 0.0);
+            sT[d][ly - fire_dy(d) + 1][lx - fire_dx(d) + 1] = T;          // slot d of the source = target - offset(d)
+            fsum += (float)T * 2.3283064365386963e-10f;
         }
-        out[0] = make_uint4(T[0], T[1], T[2], T[3]);
-        out[1] = make_uint4(T[4], T[5], T[6], T[7]);
-        out += cells * 2;
+        // scheduling hint only (never enters a result): sum of the contagion probabilities of this parameter vector
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) fsum += __shfl_xor_sync(0xFFFFFFFFu, fsum, o);
+        if (lx == 0) atomicAdd(&s_mean[q], fsum);
+        __syncthreads();
+        uint32_t* const tp = thr + (size_t)(p0 + q) * cells * 8;
+        if (inside) {                                                     // own cell as a source
+            uint32_t* const out = tp + c * 8;
+            if (lx >= 1 && lx <= kThrTX - 2 && ly >= 1 && ly <= kThrTY - 2) {
+                reinterpret_cast<uint4*>(out)[0] = make_uint4(sT[0][ly + 1][lx + 1], sT[1][ly + 1][lx + 1], sT[2][ly + 1][lx + 1], sT[3][ly + 1][lx + 1]);
+                reinterpret_cast<uint4*>(out)[1] = make_uint4(sT[4][ly + 1][lx + 1], sT[5][ly + 1][lx + 1], sT[6][ly + 1][lx + 1], sT[7][ly + 1][lx + 1]);
+            } else {
+#pragma unroll
+                for (int d = 0; d < 8; ++d) {
+                    const int tx = lx + fire_dx(d), ty = ly + fire_dy(d);
+                    if (tx >= 0 && tx < kThrTX && ty >= 0 && ty < kThrTY) out[d] = sT[d][ly + 1][lx + 1];
+                }
+            }
+        }
+        if (hx != -2) {                                                   // one cell of the ring around the tile
+            const int gx = x0 + hx, gy = y0 + hy;
+            if (gx >= 0 && gx < W && gy >= 0 && gy < H) {
+                uint32_t* const out = tp + ((size_t)gy * W + gx) * 8;
+#pragma unroll
+                for (int d = 0; d < 8; ++d) {
+                    const int tx = hx + fire_dx(d), ty = hy + fire_dy(d);
+                    if (tx >= 0 && tx < kThrTX && ty >= 0 && ty < kThrTY) out[d] = sT[d][hy + 1][hx + 1];
+                }
+            }
+        }
+        __syncthreads();
     }
+    if (tid < np) atomicAdd(param_mean + p0 + tid, s_mean[tid]);
+}
+
+// Test hook: the table of one parameter vector in TARGET-indexed form out[c][d] = T(target c, direction d).
+// Entries whose source c - offset(d) lies outside the lattice are in no sector; they are evaluated here by the
+// same device function.
+__global__ void __launch_bounds__(256)
+fire_thresholds_gather_kernel(const float* __restrict__ beta5, int W, int H,
+                              const uint8_t* __restrict__ flags, const uint8_t* __restrict__ uphill,
+                              const double* __restrict__ psi, const double* __restrict__ tan_slope,
+                              const double* __restrict__ omega, const uint32_t* __restrict__ thr_p, uint32_t* __restrict__ out)
+{
+    const size_t cells = (size_t)W * H;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // one thread per (cell, d)
+    if (i >= cells * 8) return;
+    const size_t c = i >> 3;
+    const int d = (int)(i & 7), x = (int)(c % W), y = (int)(c / W);
+    const int sx = x - fire_dx(d), sy = y - fire_dy(d);
+    uint32_t T;
+    if (sx >= 0 && sx < W && sy >= 0 && sy < H) {
+        T = thr_p[((size_t)sy * W + sx) * 8 + d];
+    } else {
+        const uint32_t f = flags[c];
+        T = 0u;
+        if (f & 1u)
+            T = fire_threshold((double)beta5[0], (double)beta5[1], (double)beta5[2], (double)beta5[3], (double)beta5[4],
+                               (f & 2u) ? 1.0 : 0.0, psi[c], omega[(size_t)d * cells + c], ((uphill[c] >> d) & 1u) ? tan_slope[c] : 0.0);
+    }
+    out[i] = T;
 }
 
 }  // namespace
@@ -128,6 +213,7 @@ extern "C" int fire_landscape_destroy(fire_landscape* L)
         cudaDeviceSynchronize();
         void* ptrs[] = { L->flags, L->uphill, L->psi, L->tan_slope, L->omega, L->burnable, L->thr, L->beta_dev,
                          L->work_counter, L->status, L->spill, L->rescue_planes, L->ref_area, L->counts_scratch,
+                         L->burnable_tiles, L->tiles, L->order, L->param_mean,
                          L->gen_buf };
         for (void* p : ptrs) if (p) cudaFree(p);
         if (L->prof_ev[0]) for (int i = 0; i < 2 * 64; ++i) if (L->prof_ev[i]) cudaEventDestroy(L->prof_ev[i]);
@@ -149,6 +235,7 @@ extern "C" int fire_landscape_create(fire_landscape** out, const uint8_t* veg, c
     if (L == nullptr) return FIRE_ENOMEM;
     L->device = dev;
     L->W = W; L->H = H; L->Ww = (W + 31) / 32; L->cells = (size_t)W * H;
+    L->Tw = (W + 7) / 8; L->Th = (H + 7) / 8;
     int sms = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
         (void)cudaGetLastError(); delete L; return FIRE_ECUDA;
@@ -187,10 +274,23 @@ extern "C" int fire_params_upload(fire_landscape* L, const float* beta, int32_t 
         int rc = fire_reserve(L, (void**)&L->thr, &L->thr_capacity, bytes);
         if (rc != FIRE_OK) return rc;
     }
-    const int block = 128;
-    dim3 grid((unsigned)((L->cells + block - 1) / block), (unsigned)((P + FIRE_THR_PGROUP - 1) / FIRE_THR_PGROUP));
-    fire_thresholds_kernel<<<grid, block, 0, (cudaStream_t)stream>>>(beta, P, L->cells, L->flags, L->uphill, L->psi,
-                                                                      L->tan_slope, L->omega, L->thr);
+    if (L->beta_capacity < (size_t)P * 5 * sizeof(float)) {
+        FIRE_CUDA_TRY(L, cudaStreamSynchronize((cudaStream_t)stream));
+        int rc = fire_reserve(L, (void**)&L->beta_dev, &L->beta_capacity, (size_t)P * 5 * sizeof(float));
+        if (rc != FIRE_OK) return rc;
+    }
+    // the handle keeps its own copy of beta (fire_thresholds_download evaluates the lattice-edge entries from it)
+    FIRE_CUDA_TRY(L, cudaMemcpyAsync(L->beta_dev, beta, (size_t)P * 5 * sizeof(float), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    if (L->param_mean_capacity < (size_t)P * sizeof(float)) {
+        FIRE_CUDA_TRY(L, cudaStreamSynchronize((cudaStream_t)stream));
+        int rc = fire_reserve(L, (void**)&L->param_mean, &L->param_mean_capacity, (size_t)P * sizeof(float));
+        if (rc != FIRE_OK) return rc;
+    }
+    FIRE_CUDA_TRY(L, cudaMemsetAsync(L->param_mean, 0, (size_t)P * sizeof(float), (cudaStream_t)stream));
+    const int tiles_x = (L->W + kThrTX - 1) / kThrTX, tiles_y = (L->H + kThrTY - 1) / kThrTY;
+    dim3 grid((unsigned)(tiles_x * tiles_y), (unsigned)((P + FIRE_THR_PGROUP - 1) / FIRE_THR_PGROUP));
+    fire_thresholds_kernel<<<grid, kThrTX * kThrTY, 0, (cudaStream_t)stream>>>(L->beta_dev, P, L->W, L->H, tiles_x, L->flags,
+                                                                                L->uphill, L->psi, L->tan_slope, L->omega, L->thr, L->param_mean);
     L->launches += 1;
     FIRE_CUDA_TRY(L, cudaGetLastError());
     L->P = P;
@@ -204,7 +304,11 @@ extern "C" int fire_thresholds_download(fire_landscape* L, int32_t p, uint32_t* 
     if (L->P == 0 || p < 0 || p >= L->P) return FIRE_ESTATE;
     fire_device_guard g(L->device);
     if (!g.ok) return FIRE_ECUDA;
-    FIRE_CUDA_TRY(L, cudaMemcpyAsync(out, L->thr + (size_t)p * L->cells * 8, L->cells * 32, cudaMemcpyDeviceToDevice,
-                                     (cudaStream_t)stream));
+    const size_t n = L->cells * 8;
+    fire_thresholds_gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
+        L->beta_dev + (size_t)p * 5, L->W, L->H, L->flags, L->uphill, L->psi, L->tan_slope, L->omega,
+        L->thr + (size_t)p * L->cells * 8, out);
+    L->launches += 1;
+    FIRE_CUDA_TRY(L, cudaGetLastError());
     return FIRE_OK;
 }

@@ -5,59 +5,52 @@
 // step, :100/:135 the run ends when the fire stops by itself; C-4):
 //   t = 0: burning = burned = {ignition} if it is inside the lattice and burnable.
 //   step t: for every burning cell b and direction d, target c = b + offset(d); if c is inside the
-//   lattice, burnable and not burned at time t: one trial rnd(seed, sim, t, c, d) against T[p][c][d].
+//   lattice, burnable and not burned at time t: one trial rnd(seed, sim, t, c, d) against T(c, d).
 //   new = targets with >= 1 success; burned |= new; burning = new.
 //
 // Design: one persistent CTA per simulation, simulations handed out by a device
-// counter, all CA steps inside ONE launch, no host round trip and no grid-wide barrier.  State per
-// simulation = ONE bit plane, the SUSCEPTIBLE plane  sus = burnable & ~burned  (it lives in the caller's
-// output buffer: fire_init_planes_kernel fills it with `burnable`, fire_finish_planes_kernel turns it
-// into the burnt map  burnable & ~sus  at the end), plus a CELL-LEVEL FRONTIER LIST of the burning
-// cells, so work is proportional to the number of trials and idle lattice is never touched.  A step:
-//   phase 1  one lane per burning cell: three words of `sus` give the 3 x 3 susceptibility window; the
-//            (target, direction) pairs of the warp are compacted into the trial queue (warp prefix sum,
-//            unrolled predicated stores, one shared atomic per warp);
+// counter (largest expected first), all CA steps inside ONE launch, no host round trip and no grid-wide
+// barrier.  State per simulation = ONE bit plane, the SUSCEPTIBLE plane  sus = burnable & ~burned,
+// stored as 8 x 8-cell tiles (one u64 per tile, so that the 3 x 3 window of a burning cell is one
+// word for 56 % of the cells), plus a CELL-LEVEL FRONTIER LIST of the burning cells: work is
+// proportional to the number of trials and idle lattice is never touched.  Thresholds are
+// SOURCE-indexed: the 8 outgoing trials of a burning cell are one 32 B sector, read exactly once in
+// the one step the cell burns.  A step:
+//   phase 1  one lane per burning cell: its tile (and up to 3 neighbouring tiles) give the 3 x 3
+//            susceptibility window, one 32 B load gives the 8 thresholds; the (target, direction,
+//            threshold) triples of the warp are compacted into the trial queue in shared memory;
 //   -- barrier: every read of `sus` for step t happens before any update of step t (synchronous update)
-//   phase 2  one lane per trial, four trials per lane in flight: one 4 B threshold load (the 32 B sector
-//            of a target cell holds its 8 directions), one Philox4x32-10 call with the round keys of the
-//            simulation held in registers, one compare; a success clears the target's bit with
-//            atomicAnd, and the lane whose atomic saw the bit still set owns the new burning cell and
-//            appends it to the next frontier (ballot / popc compaction, one shared atomic per warp).
+//   phase 2  one lane per trial: one Philox4x32-10 call, one compare; a success clears the target's
+//            bit with atomicAnd, and the lane whose atomic saw the bit still set owns the new burning
+//            cell and appends it to the next frontier (ballot / popc compaction).
 //   -- barrier
-// Lists live in shared memory and continue in a per-CTA global spill area (coalesced); if the frontier
-// outgrows even that, the simulation is handed to the rescue kernel below: a plain full-sweep,
-// three-plane, pull-style restatement of the same rules with no lists at all.
+// Lists live in shared memory and continue in a per-CTA global spill area; if the frontier outgrows
+// even that, the simulation is handed to the rescue kernel below: a plain full-sweep, three-plane,
+// pull-style restatement of the same rules with no lists at all.
 #include "fire_internal.cuh"
 
 namespace {
 
 struct prop_params {
     const uint32_t* burnable;     // [H][Ww]
-    const uint32_t* thr;          // [P][cells][8]
+    const uint32_t* thr;          // [P][cells][8], source-indexed
     const int32_t*  ignitions;    // [S][2]
     const int32_t*  sim_param;    // [S]
     const uint64_t* seeds;        // [S]
     const int32_t*  sim_ids;      // [S] or null
-    uint32_t* out_burned;         // [S][H][Ww]: the susceptible plane while the fast kernel runs
+    const uint32_t* order;        // [S] launch order or null
+    uint64_t* tiles;              // [S][Th][Tw] susceptible planes
+    uint32_t* out_burned;         // [S][H][Ww]
     uint32_t* out_steps;          // [S] or null
     unsigned long long* out_trials;  // [S] or null
     unsigned int* work_counter;   // [0] next sim of the fast kernel, [1] number of sims handed to the rescue kernel
     uint32_t* rescue_list;        // [S]
-    uint32_t* spill;              // [grid][2 * (capA - capA_s) + (capQ - capQ_s)]
-    int S, P, W, H, Ww;
+    uint32_t* spill;              // [grid][2 * (capQ - capQ_s) + 2 * (capA - capA_s)]
+    int S, P, W, H, Ww, Tw, Th;
     uint32_t max_steps;
     uint32_t capA_s, capQ_s;      // shared-memory entries: each frontier list, the trial queue
     uint32_t capA, capQ;          // total entries (shared + spill); capQ >= 8 * capA
 };
-
-__device__ __forceinline__ uint32_t list_get(const uint32_t* s, const uint32_t* g, uint32_t cap_s, uint32_t i)
-{
-    return i < cap_s ? s[i] : __ldcg(g + (i - cap_s));
-}
-__device__ __forceinline__ void list_put(uint32_t* s, uint32_t* g, uint32_t cap_s, uint32_t i, uint32_t v)
-{
-    if (i < cap_s) s[i] = v; else __stcg(g + (i - cap_s), v);
-}
 
 __device__ __forceinline__ uint32_t lanemask_lt()
 {
@@ -65,35 +58,33 @@ __device__ __forceinline__ uint32_t lanemask_lt()
 }
 
 // Frontier entry: (y << 16) | x.  Trial item: (ty << 16) | (tx << 3) | d  (x, y < 8192).
-// Item of the trial "burning cell e spreads in direction d": item(e) + kItemDelta(d).
+// Item of the trial "burning cell e spreads in direction d": item(e) + item_delta(d).
 __device__ __forceinline__ uint32_t item_delta(int d)
 {
     return (uint32_t)(fire_dy(d) * 65536 + fire_dx(d) * 8 + d);
 }
 
-// Window of three susceptibility bits (x-1, x, x+1) -> bits 0..2, from the word holding x and, at the
-// word's ends, bit 31 of the word to the left / bit 0 of the word to the right.
-__device__ __forceinline__ uint32_t win3(uint32_t mid, uint32_t lft, uint32_t rgt, int bx)
+// Threshold sector of a burning cell: read once, so keep it out of L1; the neighbouring sectors (the next
+// cells of the same row) are what the front reaches next, so let L2 fetch them with the miss.
+__device__ __forceinline__ uint4 ldg_thr(const uint4* p)
 {
-    return (bx ? __funnelshift_r(mid, rgt, bx - 1) : ((mid << 1) | (lft >> 31))) & 7u;
-}
-
-// Threshold load: read-only path, and ask L2 to fetch the whole 256 B around a miss (the thresholds of the 8
-// x-adjacent cells): HBM serves a random 32 B sector and a random 256 B chunk at nearly the same rate, and the
-// neighbours are the next cells the front reaches.
-__device__ __forceinline__ uint32_t ldg_thr(const uint32_t* p)
-{
-    uint32_t v;
-#ifndef FIRE_NO_L2_PREFETCH
-    asm volatile("ld.global.nc.L2::256B.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    uint4 v;
+#if defined(FIRE_THR_L2_256)
+    asm volatile("ld.global.nc.L1::no_allocate.L2::256B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+#elif defined(FIRE_THR_L2_PLAIN)
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
 #else
-    v = __ldg(p);
+    asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
 #endif
     return v;
 }
 
+__device__ __forceinline__ uint64_t ldcg_u64(const uint64_t* p) { return (uint64_t)__ldcg(reinterpret_cast<const unsigned long long*>(p)); }
+
 constexpr int kTrialsInFlight = 4;   // trials per lane issued together in phase 2
 constexpr int kCellsInFlight = 2;    // burning cells per lane issued together in phase 1
+constexpr uint32_t kM0 = 0xD2511F53u, kM1 = 0xCD9E8D57u;       // Philox4x32 multipliers
+constexpr uint32_t kW0 = 0x9E3779B9u, kW1 = 0xBB67AE85u;       // Philox key bumps (Weyl constants)
 
 // ------------------------------------------------------------------------------------------------
 // Fast kernel: one persistent CTA per simulation.
@@ -105,56 +96,53 @@ constexpr int kCellsInFlight = 2;    // burning cells per lane issued together i
 __global__ void __launch_bounds__(FIRE_LB_THREADS, FIRE_LB_CTAS)
 fire_propagate_kernel(const prop_params prm)
 {
-    extern __shared__ uint32_t smem[];
+    extern __shared__ __align__(16) uint32_t smem[];
     const uint32_t capA_s = prm.capA_s, capQ_s = prm.capQ_s;
-    uint32_t* const As0 = smem;
+    uint2* const Qs = reinterpret_cast<uint2*>(smem);
+    uint32_t* const As0 = smem + 2 * (size_t)capQ_s;
     uint32_t* const As1 = As0 + capA_s;
-    uint32_t* const Qs = As1 + capA_s;
-    const size_t spill_per_cta = (size_t)2 * (prm.capA - capA_s) + (prm.capQ - capQ_s);
-    uint32_t* const Ag0 = prm.spill + (size_t)blockIdx.x * spill_per_cta;
+    const size_t spill_per_cta = (size_t)2 * (prm.capQ - capQ_s) + (size_t)2 * (prm.capA - capA_s);
+    uint2* const Qg = reinterpret_cast<uint2*>(prm.spill + (size_t)blockIdx.x * spill_per_cta);
+    uint32_t* const Ag0 = prm.spill + (size_t)blockIdx.x * spill_per_cta + (size_t)2 * (prm.capQ - capQ_s);
     uint32_t* const Ag1 = Ag0 + (prm.capA - capA_s);
-    uint32_t* const Qg = Ag1 + (prm.capA - capA_s);
 
     __shared__ unsigned int s_sim, s_cntA[2], s_cntQ[2], s_over;
     __shared__ unsigned long long s_trials;
 
     const int tid = threadIdx.x, lane = tid & 31, nthr = blockDim.x;
-    const int W = prm.W, H = prm.H, Ww = prm.Ww;
+    const int W = prm.W, H = prm.H, Tw = prm.Tw, Th = prm.Th;
     const uint32_t lt = lanemask_lt();
 
     for (;;) {
         __syncthreads();                       // the previous simulation's last reads of s_* are done
-        if (tid == 0) s_sim = atomicAdd(prm.work_counter, 1u);
+        if (tid == 0) {
+            const unsigned int k = atomicAdd(prm.work_counter, 1u);
+            s_sim = (k < (unsigned int)prm.S) ? (prm.order ? prm.order[k] : k) : 0xFFFFFFFFu;
+        }
         __syncthreads();
         const uint32_t s = s_sim;
-        if (s >= (uint32_t)prm.S) break;
-#ifdef FIRE_TRACE
-        unsigned long long trace_t0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t0));
-#endif
+        if (s == 0xFFFFFFFFu) break;
 
         const int p = prm.sim_param[s];
         const int ix = prm.ignitions[2 * s], iy = prm.ignitions[2 * s + 1];
         const uint64_t seed = prm.seeds[s];
         const uint32_t sim = prm.sim_ids ? (uint32_t)prm.sim_ids[s] : s;
-        uint32_t* const sus = prm.out_burned + (size_t)s * H * Ww;
+        uint64_t* const sus = prm.tiles + (size_t)s * Tw * Th;
+        uint32_t* const sus32 = reinterpret_cast<uint32_t*>(sus);
         bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < W && iy >= 0 && iy < H;     // R-12
-        if (valid) valid = (__ldg(prm.burnable + (size_t)iy * Ww + (ix >> 5)) >> (ix & 31)) & 1u;
+        if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
         const uint32_t* const thr = prm.thr + (valid ? (size_t)p * W * H * 8 : 0);
-
-        // round keys of Philox4x32-10 for this simulation's seed (bumped before every round but the first)
-        uint32_t rk0[10], rk1[10];
-#pragma unroll
-        for (int r = 0; r < 10; ++r) {
-            rk0[r] = (uint32_t)seed + (uint32_t)r * 0x9E3779B9u;
-            rk1[r] = (uint32_t)(seed >> 32) + (uint32_t)r * 0xBB67AE85u;
-        }
+        const uint32_t key_lo = (uint32_t)seed, key_hi = (uint32_t)(seed >> 32);
+        // Philox round 0 multiplies the counter word `sim` by M1: the same product for every trial of the simulation
+        const uint32_t bh = __umulhi(sim, kM1), bl = sim * kM1;
 
         if (tid == 0) {
             s_cntA[0] = valid ? 1u : 0u; s_cntA[1] = 0u; s_cntQ[0] = 0u; s_cntQ[1] = 0u;
             s_over = 0u; s_trials = 0ull;
             if (valid) {
-                list_put(As0, Ag0, capA_s, 0u, ((uint32_t)iy << 16) | (uint32_t)ix);
-                atomicAnd(sus + (size_t)iy * Ww + (ix >> 5), ~(1u << (ix & 31)));
+                const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
+                if (capA_s > 0) As0[0] = e0; else Ag0[0] = e0;
+                atomicAnd(sus32 + (((size_t)(iy >> 3) * Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
         }
         __syncthreads();
@@ -164,53 +152,60 @@ fire_propagate_kernel(const prop_params prm)
         bool over = false;
         while (nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
             const int par = t & 1;
-            uint32_t* const Ac_s = par ? As1 : As0;  uint32_t* const Ac_g = par ? Ag1 : Ag0;
-            uint32_t* const An_s = par ? As0 : As1;  uint32_t* const An_g = par ? Ag0 : Ag1;
+            const uint32_t* const Ac_s = par ? As1 : As0;  const uint32_t* const Ac_g = par ? Ag1 : Ag0;
+            uint32_t* const An_s = par ? As0 : As1;        uint32_t* const An_g = par ? Ag0 : Ag1;
 
-            // ---- phase 1: susceptible neighbours of the burning cells -> trial queue
-            // kCellsInFlight burning cells per lane; all their `sus` loads are issued before any is used.
+            // ---- phase 1: susceptible neighbours of the burning cells and their thresholds -> trial queue.
+            // kCellsInFlight burning cells per lane; all their loads are issued before any is used.
             for (uint32_t i0 = (uint32_t)(tid & ~31) * kCellsInFlight; i0 < nA; i0 += (uint32_t)nthr * kCellsInFlight) {
-                uint32_t e[kCellsInFlight], mid[kCellsInFlight], upw[kCellsInFlight], dnw[kCellsInFlight], m[kCellsInFlight];
+                uint32_t e[kCellsInFlight], win[kCellsInFlight];
+                uint64_t tc[kCellsInFlight], th[kCellsInFlight], tv[kCellsInFlight], td[kCellsInFlight];
+                uint4 Ta[kCellsInFlight], Tb[kCellsInFlight];
 #pragma unroll
                 for (int k = 0; k < kCellsInFlight; ++k) {
                     const uint32_t i = i0 + 32u * k + lane;
-                    e[k] = 0xFFFFFFFFu; mid[k] = 0u; upw[k] = 0u; dnw[k] = 0u;
+                    e[k] = 0xFFFFFFFFu; tc[k] = 0ull; th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
+                    Ta[k] = make_uint4(0u, 0u, 0u, 0u); Tb[k] = make_uint4(0u, 0u, 0u, 0u);
                     if (i < nA) {
-                        e[k] = list_get(Ac_s, Ac_g, capA_s, i);
-                        const uint32_t x = e[k] & 0xFFFFu, y = e[k] >> 16;
-                        const uint32_t* const r1 = sus + (y * (uint32_t)Ww + (x >> 5));
-                        mid[k] = __ldcg(r1);
-                        if (y > 0) upw[k] = __ldcg(r1 - Ww);
-                        if (y + 1 < (uint32_t)H) dnw[k] = __ldcg(r1 + Ww);
+                        e[k] = (i < capA_s) ? Ac_s[i] : __ldcg(Ac_g + (i - capA_s));
+                        const int x = (int)(e[k] & 0xFFFFu), y = (int)(e[k] >> 16);
+                        const int tx0 = x >> 3, ty0 = y >> 3, bx = x & 7, by = y & 7;
+                        const int hoff = (bx == 0 && tx0 > 0) ? -1 : ((bx == 7 && tx0 + 1 < Tw) ? 1 : 0);
+                        const int voff = (by == 0 && ty0 > 0) ? -Tw : ((by == 7 && ty0 + 1 < Th) ? Tw : 0);
+                        const uint64_t* const tp = sus + ((size_t)ty0 * Tw + tx0);
+                        const uint4* const sp = reinterpret_cast<const uint4*>(thr + ((size_t)y * W + x) * 8);
+                        tc[k] = ldcg_u64(tp);
+                        Ta[k] = ldg_thr(sp);
+                        Tb[k] = ldg_thr(sp + 1);
+                        if (hoff) th[k] = ldcg_u64(tp + hoff);
+                        if (voff) tv[k] = ldcg_u64(tp + voff);
+                        if (hoff && voff) td[k] = ldcg_u64(tp + hoff + voff);
                     }
                 }
                 uint32_t cnt = 0;
 #pragma unroll
                 for (int k = 0; k < kCellsInFlight; ++k) {
-                    m[k] = 0u;
+                    win[k] = 0u;
                     if (e[k] != 0xFFFFFFFFu) {
-                        const uint32_t x = e[k] & 0xFFFFu, y = e[k] >> 16;
-                        const int wx = (int)(x >> 5), bx = (int)(x & 31u);
-                        uint32_t l0 = 0, l1 = 0, l2 = 0, g0 = 0, g1 = 0, g2 = 0;
-                        if (bx == 0 || bx == 31) {                         // the window crosses into a neighbouring word (1 cell in 16)
-                            const uint32_t* const r1 = sus + (y * (uint32_t)Ww + (uint32_t)wx);
-                            const bool has_up = y > 0, has_dn = y + 1 < (uint32_t)H;
-                            if (bx == 0 && wx > 0) {
-                                l1 = __ldcg(r1 - 1);
-                                if (has_up) l0 = __ldcg(r1 - Ww - 1);
-                                if (has_dn) l2 = __ldcg(r1 + Ww - 1);
-                            } else if (bx == 31 && wx + 1 < Ww) {
-                                g1 = __ldcg(r1 + 1);
-                                if (has_up) g0 = __ldcg(r1 - Ww + 1);
-                                if (has_dn) g2 = __ldcg(r1 + Ww + 1);
-                            }
+                        const uint32_t bx = e[k] & 7u, by = (e[k] >> 16) & 7u;
+                        // rows y-1, y, y+1 of the cell's tile column (w3c) and of the horizontally adjacent one (w3h), one per byte
+                        const uint32_t selr = ((by + 7u) & 7u) | (by << 4) | (((by + 1u) & 7u) << 8);
+                        uint32_t w3c = __byte_perm((uint32_t)tc[k], (uint32_t)(tc[k] >> 32), selr) & 0xFFFFFFu;
+                        uint32_t w3h = __byte_perm((uint32_t)th[k], (uint32_t)(th[k] >> 32), selr) & 0xFFFFFFu;
+                        if (by == 0u) {            // row y-1 is row 7 of the tile above (or does not exist)
+                            w3c = (w3c & 0xFFFF00u) | (uint32_t)(tv[k] >> 56);
+                            w3h = (w3h & 0xFFFF00u) | (uint32_t)(td[k] >> 56);
+                        } else if (by == 7u) {     // row y+1 is row 0 of the tile below
+                            w3c = (w3c & 0x00FFFFu) | (((uint32_t)tv[k] & 0xFFu) << 16);
+                            w3h = (w3h & 0x00FFFFu) | (((uint32_t)td[k] & 0xFFu) << 16);
                         }
-                        const uint32_t up = win3(upw[k], l0, g0, bx), md = win3(mid[k], l1, g1, bx), dn = win3(dnw[k], l2, g2, bx);
-                        // bit d of m: the neighbour reached by travelling in direction d can still burn
-                        m[k] = ((up >> 1) & 3u) | (md & 4u) | ((dn & 4u) << 1) | ((dn & 2u) << 3) | ((dn & 1u) << 5) |
-                               ((md & 1u) << 6) | ((up & 1u) << 7);
+                        // per byte: bit 0 = (x-1), bit 1 = x, bit 2 = (x+1)
+                        const uint32_t tcen = (w3c << 1) >> bx;
+                        const uint32_t mC = (bx == 0u) ? 0x060606u : ((bx == 7u) ? 0x030303u : 0x070707u);
+                        const uint32_t hb = (bx == 0u) ? ((w3h >> 7) & 0x010101u) : ((w3h << 2) & 0x040404u);
+                        win[k] = (tcen & mC) | hb;
                     }
-                    cnt += __popc(m[k]);
+                    cnt += __popc(win[k]);
                 }
                 uint32_t incl = cnt;
 #pragma unroll
@@ -226,38 +221,53 @@ fire_propagate_kernel(const prop_params prm)
                 uint32_t pos = qbase + incl - cnt;
                 my_trials += cnt;
                 const bool in_shared = qbase + total <= capQ_s;           // warp-uniform: the whole batch fits in shared memory
+#define FIRE_EMIT(bit, d, Tv)                                                                          \
+                    if (w & (1u << (bit))) {                                                           \
+                        const uint32_t q = pos + __popc(w & ((1u << (bit)) - 1u));                     \
+                        const uint2 it = make_uint2(base + item_delta(d), (Tv));                       \
+                        if (in_shared || q < capQ_s) Qs[q] = it; else __stcg(Qg + (q - capQ_s), it);   \
+                    }
 #pragma unroll
                 for (int k = 0; k < kCellsInFlight; ++k) {
+                    const uint32_t w = win[k];
                     const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
-                    if (in_shared) {
-#pragma unroll
-                        for (int d = 0; d < 8; ++d)
-                            if (m[k] & (1u << d)) Qs[pos + __popc(m[k] & ((1u << d) - 1u))] = base + item_delta(d);
-                    } else {
-#pragma unroll
-                        for (int d = 0; d < 8; ++d)
-                            if (m[k] & (1u << d)) list_put(Qs, Qg, capQ_s, pos + __popc(m[k] & ((1u << d) - 1u)), base + item_delta(d));
-                    }
-                    pos += __popc(m[k]);
+                    FIRE_EMIT(0, 7, Tb[k].w)  FIRE_EMIT(1, 0, Ta[k].x)  FIRE_EMIT(2, 1, Ta[k].y)
+                    FIRE_EMIT(8, 6, Tb[k].z)  FIRE_EMIT(10, 2, Ta[k].z)
+                    FIRE_EMIT(16, 5, Tb[k].y) FIRE_EMIT(17, 4, Tb[k].x) FIRE_EMIT(18, 3, Ta[k].w)
+                    pos += __popc(w);
                 }
+#undef FIRE_EMIT
             }
             __syncthreads();
             const uint32_t nQ = s_cntQ[par];
             if (tid == 0) { s_cntA[par] = 0u; s_cntQ[par ^ 1] = 0u; }     // next step's counters; nobody reads them now
 
             // ---- phase 2: one Bernoulli trial per lane-slot, kTrialsInFlight per lane, in stages so that each
-            // long latency (threshold load, atomic) is waited for once per batch: loads -> Philox -> atomics -> compaction
+            // long latency is waited for once per batch: queue reads -> Philox -> atomics -> compaction.
+            // Philox4x32-10(counter = (c, t, sim, d >> 2), key = seed), word d & 3 (C-1).  Round keys are
+            // rebuilt here once per step (they are dead during phase 1) and made opaque so that they stay in registers.
+            uint32_t rk0[10], rk1[10];
+#pragma unroll
+            for (int r = 0; r < 10; ++r) {
+                rk0[r] = key_lo + (uint32_t)r * kW0;
+                rk1[r] = key_hi + (uint32_t)r * kW1;
+                asm volatile("" : "+r"(rk0[r]), "+r"(rk1[r]));
+            }
+            // rounds 0 and 1 see (c1, c2) = (t, sim): everything that does not depend on the cell is per-step
+            const uint32_t r0c0 = bh ^ t ^ rk0[0];                      // c0 after round 0
+            const uint32_t a1h = __umulhi(r0c0, kM0), a1l = r0c0 * kM0; // round 1: c0 * M0
+            const uint32_t x1 = bl ^ rk0[1], y1 = a1h ^ rk1[1];
             for (uint32_t j0 = (uint32_t)(tid & ~31) * kTrialsInFlight; j0 < nQ; j0 += (uint32_t)nthr * kTrialsInFlight) {
                 uint32_t item[kTrialsInFlight], T[kTrialsInFlight], old[kTrialsInFlight];
+                const bool q_shared = j0 + 32u * kTrialsInFlight <= capQ_s;     // warp-uniform
 #pragma unroll
                 for (int u = 0; u < kTrialsInFlight; ++u) {
                     const uint32_t j = j0 + 32u * u + lane;
                     item[u] = 0xFFFFFFFFu;
                     T[u] = 0u;
                     if (j < nQ) {
-                        item[u] = list_get(Qs, Qg, capQ_s, j);
-                        const uint32_t c = (item[u] >> 16) * (uint32_t)W + ((item[u] >> 3) & 0x1FFFu);
-                        T[u] = ldg_thr(thr + (c * 8u + (item[u] & 7u)));
+                        const uint2 it = (q_shared || j < capQ_s) ? Qs[j] : __ldcg(Qg + (j - capQ_s));
+                        item[u] = it.x; T[u] = it.y;
                     }
                 }
                 bool succ[kTrialsInFlight];
@@ -266,12 +276,19 @@ fire_propagate_kernel(const prop_params prm)
                     succ[u] = false;
                     if (j0 + 32u * u < nQ) {                               // warp-uniform
                         const uint32_t ty = item[u] >> 16, tx = (item[u] >> 3) & 0x1FFFu, d = item[u] & 7u;
-                        // Philox4x32-10(counter = (c, t, sim, d >> 2), key = seed), word d & 3   (C-1)
-                        uint32_t c0 = ty * (uint32_t)W + tx, c1 = t, c2 = sim, c3 = d >> 2;
+                        const uint32_t cell = ty * (uint32_t)W + tx;
+                        // round 0: (cell, t, sim, d >> 2) -> (r0c0, bl, hi(cell * M0) ^ (d >> 2) ^ k1, lo(cell * M0))
+                        uint32_t c3 = cell * kM0;
+                        uint32_t c2 = __umulhi(cell, kM0) ^ (d >> 2) ^ rk1[0];
+                        // round 1: a = r0c0 * M0 (per step), b = c2 * M1
+                        uint32_t c0 = __umulhi(c2, kM1) ^ x1;
+                        uint32_t c1 = c2 * kM1;
+                        c2 = y1 ^ c3;
+                        c3 = a1l;
 #pragma unroll
-                        for (int r = 0; r < 10; ++r) {
-                            const uint64_t a = (uint64_t)c0 * 0xD2511F53ull;
-                            const uint64_t b = (uint64_t)c2 * 0xCD9E8D57ull;
+                        for (int r = 2; r < 10; ++r) {
+                            const uint64_t a = (uint64_t)c0 * kM0;
+                            const uint64_t b = (uint64_t)c2 * kM1;
                             const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ rk0[r];
                             const uint32_t n2 = (uint32_t)(a >> 32) ^ c3 ^ rk1[r];
                             c1 = (uint32_t)b; c3 = (uint32_t)a; c0 = n0; c2 = n2;
@@ -286,14 +303,19 @@ fire_propagate_kernel(const prop_params prm)
                     old[u] = 0u;
                     if (succ[u]) {
                         const uint32_t ty = item[u] >> 16, tx = (item[u] >> 3) & 0x1FFFu;
-                        old[u] = atomicAnd(sus + (ty * (uint32_t)Ww + (tx >> 5)), ~(1u << (tx & 31u)));
+                        const uint32_t widx = (((ty >> 3) * (uint32_t)Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
+                        old[u] = atomicAnd(sus32 + widx, ~(1u << (((ty & 3u) << 3) | (tx & 7u))));
+#ifdef FIRE_PREFETCH_THR
+                        asm volatile("prefetch.global.L2 [%0];" :: "l"(thr + ((size_t)(ty * (uint32_t)W + tx)) * 8));
+#endif
                     }
                 }
                 uint32_t fresh_mask[kTrialsInFlight];
                 uint32_t n_fresh = 0;
 #pragma unroll
                 for (int u = 0; u < kTrialsInFlight; ++u) {
-                    const bool fresh = succ[u] && ((old[u] >> ((item[u] >> 3) & 31u)) & 1u);
+                    const uint32_t bit = (((item[u] >> 16) & 3u) << 3) | ((item[u] >> 3) & 7u);
+                    const bool fresh = succ[u] && ((old[u] >> bit) & 1u);
                     fresh_mask[u] = __ballot_sync(0xFFFFFFFFu, fresh);
                     n_fresh += __popc(fresh_mask[u]);
                 }
@@ -301,11 +323,14 @@ fire_propagate_kernel(const prop_params prm)
                 uint32_t abase = 0;
                 if (lane == 0) abase = atomicAdd(&s_cntA[par ^ 1], n_fresh);
                 abase = __shfl_sync(0xFFFFFFFFu, abase, 0);
+                const bool a_shared = abase + n_fresh <= capA_s;           // warp-uniform
 #pragma unroll
                 for (int u = 0; u < kTrialsInFlight; ++u) {
                     if (fresh_mask[u] & (1u << lane)) {
                         const uint32_t pos = abase + __popc(fresh_mask[u] & lt);
-                        if (pos < prm.capA) list_put(An_s, An_g, capA_s, pos, (item[u] & 0xFFFF0000u) | ((item[u] >> 3) & 0x1FFFu));
+                        const uint32_t en = (item[u] & 0xFFFF0000u) | ((item[u] >> 3) & 0x1FFFu);
+                        if (a_shared || pos < capA_s) An_s[pos] = en;
+                        else if (pos < prm.capA) __stcg(An_g + (pos - capA_s), en);
                         else s_over = 1u;
                     }
                     abase += __popc(fresh_mask[u]);
@@ -326,43 +351,100 @@ fire_propagate_kernel(const prop_params prm)
             } else {
                 if (prm.out_steps) prm.out_steps[s] = t;
                 if (prm.out_trials) prm.out_trials[s] = s_trials;
-#ifdef FIRE_TRACE   // diagnostic build only: out_trials = (start us << 32) | duration us of this simulation, for schedule plots
-                unsigned long long trace_t1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t1));
-                if (prm.out_trials) prm.out_trials[s] = (((trace_t0 / 1000ull) & 0xFFFFFFFFull) << 32) | (((trace_t1 - trace_t0) / 1000ull) & 0xFFFFFFFFull);
-#endif
             }
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// Plane set-up and tear-down around the fast kernel: sus = burnable before, burnt = burnable & ~sus after.
-// Pure streams over S planes; grid = (chunks of the plane, S).
+// Plane set-up and tear-down around the fast kernel (pure streams).
+//   fire_burnable_tiles_kernel : once per landscape, burnable bitmap -> tile layout
+//   fire_init_tiles_kernel     : sus = burnable for every simulation of the batch
+//   fire_finish_kernel         : burnt map (row-major bitmap) = burnable & ~sus
 // ------------------------------------------------------------------------------------------------
-template <bool kFinish>
 __global__ void __launch_bounds__(256)
-fire_planes_kernel(const uint32_t* __restrict__ burnable, uint32_t* __restrict__ planes, size_t nw, int vec4)
+fire_burnable_tiles_kernel(const uint32_t* __restrict__ burnable, int H, int Ww, int Tw, int Th, uint64_t* __restrict__ out)
 {
-    uint32_t* const plane = planes + (size_t)blockIdx.y * nw;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Tw * Th) return;
+    const int ty = i / Tw, tx = i % Tw;
+    uint64_t tile = 0ull;
+    for (int r = 0; r < 8; ++r) {
+        const int y = ty * 8 + r;
+        if (y < H) tile |= (uint64_t)((burnable[(size_t)y * Ww + (tx >> 2)] >> ((tx & 3) * 8)) & 0xFFu) << (8 * r);
+    }
+    out[i] = tile;
+}
+
+__global__ void __launch_bounds__(256)
+fire_init_tiles_kernel(const uint64_t* __restrict__ burnable_tiles, uint64_t* __restrict__ tiles, size_t nt)
+{
+    uint64_t* const plane = tiles + (size_t)blockIdx.y * nt;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
-    if (vec4) {
-        const uint4* const b4 = reinterpret_cast<const uint4*>(burnable);
+    if ((nt & 1) == 0) {
+        const uint4* const b4 = reinterpret_cast<const uint4*>(burnable_tiles);
         uint4* const p4 = reinterpret_cast<uint4*>(plane);
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nw / 4; i += stride) {
-            uint4 b = __ldg(b4 + i);
-            if (kFinish) {
-                const uint4 s = __ldcs(p4 + i);
-                b.x &= ~s.x; b.y &= ~s.y; b.z &= ~s.z; b.w &= ~s.w;
-            }
-            p4[i] = b;
-        }
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nt / 2; i += stride) p4[i] = __ldg(b4 + i);
     } else {
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nw; i += stride) {
-            uint32_t b = __ldg(burnable + i);
-            if (kFinish) b &= ~__ldcs(plane + i);
-            plane[i] = b;
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += stride) plane[i] = __ldg(burnable_tiles + i);
+    }
+}
+
+// one thread per (tile row, bitmap word column): 4 tiles in (32 B), 8 words out (one per lattice row)
+__global__ void __launch_bounds__(256)
+fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __restrict__ tiles, uint32_t* __restrict__ out_burned,
+                   int H, int Ww, int Tw, int Th)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= Th * Ww) return;
+    const int ty = i / Ww, wx = i % Ww;
+    const uint64_t* const row = tiles + (size_t)blockIdx.y * Tw * Th + (size_t)ty * Tw;
+    uint64_t tl[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) tl[k] = (4 * wx + k < Tw) ? __ldcs(reinterpret_cast<const unsigned long long*>(row + 4 * wx + k)) : 0ull;
+    uint32_t* const out = out_burned + (size_t)blockIdx.y * H * Ww;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int y = ty * 8 + r;
+        if (y < H) {
+            uint32_t susw = 0u;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) susw |= (uint32_t)((tl[k] >> (8 * r)) & 0xFFull) << (8 * k);
+            const size_t wi = (size_t)y * Ww + wx;
+            out[wi] = __ldg(burnable + wi) & ~susw;
         }
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Launch order: simulations sorted by the mean contagion probability of their parameter vector,
+// largest first (a counting sort on a 10-bit key).  Burn sizes are heavy-tailed
+// (PAPER.md:135, :211): starting the large fires first lets the small ones fill the tail of the launch.
+// ------------------------------------------------------------------------------------------------
+constexpr int kOrderBuckets = 1024;
+__global__ void __launch_bounds__(1024)
+fire_order_kernel(const int32_t* __restrict__ sim_param, const float* __restrict__ param_mean, int S, int P, float scale, uint32_t* __restrict__ order)
+{
+    __shared__ unsigned int hist[kOrderBuckets];
+    __shared__ unsigned int start[kOrderBuckets];
+    const int tid = threadIdx.x;
+    for (int b = tid; b < kOrderBuckets; b += blockDim.x) hist[b] = 0u;
+    __syncthreads();
+    auto bucket_of = [&](int s) -> int {
+        const int p = sim_param[s];
+        float m = (p >= 0 && p < P) ? param_mean[p] * scale : 0.0f;
+        m = fminf(fmaxf(m, 0.0f), 1.0f);
+        return (kOrderBuckets - 1) - (int)(m * (float)(kOrderBuckets - 1));     // bucket 0 = largest mean
+    };
+    for (int s = tid; s < S; s += blockDim.x) atomicAdd(&hist[bucket_of(s)], 1u);
+    __syncthreads();
+    if (tid == 0) {
+        unsigned int acc = 0u;
+        for (int b = 0; b < kOrderBuckets; ++b) { start[b] = acc; acc += hist[b]; }
+    }
+    __syncthreads();
+    // order inside a bucket is whatever the atomics give: it only decides scheduling, never results
+    for (int s = tid; s < S; s += blockDim.x) order[atomicAdd(&start[bucket_of(s)], 1u)] = (uint32_t)s;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -444,7 +526,7 @@ fire_propagate_rescue_kernel(const prop_params prm, uint32_t* planes)
                     for (int d = 0; d < 8; ++d) {
                         if (((src[d] >> bx) & 1u) == 0u) continue;
                         ++my_trials;
-                        const uint32_t T = __ldg(thr + (size_t)c * 8 + d);
+                        const uint32_t T = __ldg(thr + (size_t)(c - (uint32_t)(fire_dy(d) * W + fire_dx(d))) * 8 + d);   // slot d of the source cell
                         hit |= fire_trial(fire_rnd(key_lo, key_hi, sim, t, c, d), T);
                     }
                     if (hit) fresh |= 1u << bx;
@@ -532,16 +614,18 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     prm.capA_s = capA_s; prm.capA = capA;
     prm.capQ = 8u * capA;
     prm.capQ_s = 2u * capA_s < prm.capQ ? 2u * capA_s : prm.capQ;
-    const size_t smem = ((size_t)2 * prm.capA_s + prm.capQ_s) * sizeof(uint32_t);
+    const size_t smem = ((size_t)2 * prm.capA_s + (size_t)2 * prm.capQ_s) * sizeof(uint32_t);
     if (smem > 200 * 1024) return FIRE_EINVAL;
 
     // ---- scratch owned by the handle (grow-only; growing waits for the stream first)
-    const size_t spill_per_cta = (size_t)2 * (prm.capA - prm.capA_s) + (prm.capQ - prm.capQ_s);
+    const size_t spill_per_cta = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);
     const size_t spill_bytes = spill_per_cta * (size_t)grid * 4 + 16;
     const size_t nw = (size_t)L->H * L->Ww;
-    const size_t plane_bytes = nw * 4;
-    const size_t rescue_bytes = plane_bytes * 2 * kRescueCtas;
-    if (L->status_capacity < (size_t)S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes) {
+    const size_t nt = (size_t)L->Tw * L->Th;
+    const size_t rescue_bytes = nw * 4 * 2 * kRescueCtas;
+    const size_t tiles_bytes = nt * 8 * (size_t)S;
+    if (L->status_capacity < (size_t)S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes ||
+        L->tiles_capacity < tiles_bytes || L->order_capacity < (size_t)S * 4 || L->burnable_tiles == nullptr) {
         FIRE_CUDA_TRY(L, cudaStreamSynchronize(st));
         size_t cap_bytes = L->status_capacity * 4;
         int rc = fire_reserve(L, (void**)&L->status, &cap_bytes, (size_t)S * 4);
@@ -549,28 +633,51 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         L->status_capacity = cap_bytes / 4;
         rc = fire_reserve(L, (void**)&L->spill, &L->spill_capacity, spill_bytes);
         if (rc != FIRE_OK) return rc;
+        rc = fire_reserve(L, (void**)&L->tiles, &L->tiles_capacity, tiles_bytes);
+        if (rc != FIRE_OK) return rc;
+        rc = fire_reserve(L, (void**)&L->order, &L->order_capacity, (size_t)S * 4);
+        if (rc != FIRE_OK) return rc;
         if (L->rescue_capacity < rescue_bytes) {
             rc = fire_reserve(L, (void**)&L->rescue_planes, &L->rescue_capacity, rescue_bytes);
             if (rc != FIRE_OK) return rc;
             FIRE_CUDA_TRY(L, cudaMemsetAsync(L->rescue_planes, 0, rescue_bytes, st));
         }
+        if (L->burnable_tiles == nullptr) {
+            size_t cap = 0;
+            rc = fire_reserve(L, (void**)&L->burnable_tiles, &cap, nt * 8);
+            if (rc != FIRE_OK) return rc;
+            fire_burnable_tiles_kernel<<<(unsigned)((nt + 255) / 256), 256, 0, st>>>(L->burnable, L->H, L->Ww, L->Tw, L->Th, L->burnable_tiles);
+            FIRE_CUDA_TRY(L, cudaGetLastError());
+            L->launches += 1;
+        }
     }
 
     prm.burnable = L->burnable; prm.thr = L->thr;
     prm.ignitions = ignitions; prm.sim_param = sim_param; prm.seeds = seeds; prm.sim_ids = sim_ids;
+    prm.tiles = L->tiles;
     prm.out_burned = out_burned; prm.out_steps = out_steps; prm.out_trials = (unsigned long long*)out_trials;
     prm.work_counter = L->work_counter; prm.rescue_list = L->status; prm.spill = L->spill;
-    prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.max_steps = max_steps;
+    prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.Tw = L->Tw; prm.Th = L->Th;
+    prm.max_steps = max_steps;
 
-    // ---- planes: sus = burnable, then the simulations, then burnt = burnable & ~sus
-    const int vec4 = (nw % 4 == 0 && ((uintptr_t)out_burned & 15u) == 0) ? 1 : 0;
-    const size_t units = vec4 ? nw / 4 : nw;
-    unsigned chunks = (unsigned)((units + 256 * 4 - 1) / (256 * 4));
-    if (chunks < 1) chunks = 1;
-    if (chunks > 64) chunks = 64;
-    const dim3 plane_grid(chunks, (unsigned)S);
-    fire_planes_kernel<false><<<plane_grid, 256, 0, st>>>(L->burnable, out_burned, nw, vec4);
-    FIRE_CUDA_TRY(L, cudaGetLastError());
+    // ---- launch order: largest expected fires first (only matters when there are more simulations than resident CTAs)
+    prm.order = nullptr;
+    if (S > grid && L->param_mean != nullptr) {
+        fire_order_kernel<<<1, 1024, 0, st>>>(sim_param, L->param_mean, S, L->P, 1.0f / ((float)L->cells * 8.0f), L->order);
+        FIRE_CUDA_TRY(L, cudaGetLastError());
+        L->launches += 1;
+        prm.order = L->order;
+    }
+
+    // ---- planes: sus = burnable (tile layout), then the simulations, then burnt = burnable & ~sus (row-major bitmap)
+    {
+        const size_t units = (nt & 1) ? nt : nt / 2;
+        unsigned chunks = (unsigned)((units + 256 * 4 - 1) / (256 * 4));
+        if (chunks < 1) chunks = 1;
+        if (chunks > 64) chunks = 64;
+        fire_init_tiles_kernel<<<dim3(chunks, (unsigned)S), 256, 0, st>>>(L->burnable_tiles, L->tiles, nt);
+        FIRE_CUDA_TRY(L, cudaGetLastError());
+    }
     FIRE_CUDA_TRY(L, cudaMemsetAsync(L->work_counter, 0, 2 * sizeof(unsigned int), st));
     if (smem > 48 * 1024)
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(fire_propagate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -579,8 +686,12 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     fire_propagate_kernel<<<grid, threads, smem, st>>>(prm);
     FIRE_CUDA_TRY(L, cudaGetLastError());
     if (prof) { FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count + 1], st)); L->prof_count += 1; }
-    fire_planes_kernel<true><<<plane_grid, 256, 0, st>>>(L->burnable, out_burned, nw, vec4);
-    FIRE_CUDA_TRY(L, cudaGetLastError());
+    {
+        const size_t n = (size_t)L->Th * L->Ww;
+        fire_finish_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)S), 256, 0, st>>>(L->burnable, L->tiles, out_burned,
+                                                                                          L->H, L->Ww, L->Tw, L->Th);
+        FIRE_CUDA_TRY(L, cudaGetLastError());
+    }
     fire_propagate_rescue_kernel<<<kRescueCtas, 256, 0, st>>>(prm, L->rescue_planes);
     FIRE_CUDA_TRY(L, cudaGetLastError());
     L->launches += 4;
