@@ -216,6 +216,14 @@ def run_ours(args) -> None:
 
     L = lf.fire_landscape_create(dev(ls["veg"]), dev(ls["slope"]), dev(ls["aspect"]), dev(ls["wind"]))
     H, Ww = L.H, L.Ww
+    if os.environ.get("FIRE_GEOM"):                      # tuning runs only: "threads,ctas_per_sm"
+        th, per = (int(v) for v in os.environ["FIRE_GEOM"].split(","))
+        lf.fire_set_launch_geometry(L, th, per)
+    if os.environ.get("FIRE_LIST"):                      # tuning runs only: "shared_entries,total_entries"
+        a, b = (int(v) for v in os.environ["FIRE_LIST"].split(","))
+        lf.fire_set_list_capacity(L, a, b)
+    if os.environ.get("FIRE_SCHEDULE"):
+        lf.fire_set_schedule(L, int(os.environ["FIRE_SCHEDULE"]))
     d_beta_ref = dev(w.ref_beta[None, :])
     d_beta = dev(w.betas)
     d_ign, d_par, d_seed, d_ids = dev(w.ignitions), dev(w.sim_param), dev(seeds_np), dev(sim_ids_np)

@@ -132,6 +132,11 @@ int fire_set_launch_geometry(fire_landscape* L, int32_t threads_per_cta, int32_t
  * rescue kernel.  Results never depend on these values.  0 = default. */
 int fire_set_list_capacity(fire_landscape* L, int32_t shared_entries, int32_t total_entries);
 
+/* Tuning knob / test hook (pin P-9): order in which the simulations of a batch are handed to the resident
+ * CTAs.  0 = default: largest expected fires first (by the mean contagion probability of their parameter
+ * vector, a by-product of fire_params_upload); 1 = batch order.  Results never depend on it. */
+int fire_set_schedule(fire_landscape* L, int32_t mode);
+
 const char* fire_error_string(int code);
 
 #ifdef __cplusplus

@@ -81,37 +81,268 @@ __device__ __forceinline__ uint4 ldg_thr(const uint4* p)
 
 __device__ __forceinline__ uint64_t ldcg_u64(const uint64_t* p) { return (uint64_t)__ldcg(reinterpret_cast<const unsigned long long*>(p)); }
 
-constexpr int kTrialsInFlight = 4;   // trials per lane issued together in phase 2
-constexpr int kCellsInFlight = 2;    // burning cells per lane issued together in phase 1
 constexpr uint32_t kM0 = 0xD2511F53u, kM1 = 0xCD9E8D57u;       // Philox4x32 multipliers
 constexpr uint32_t kW0 = 0x9E3779B9u, kW1 = 0xBB67AE85u;       // Philox key bumps (Weyl constants)
 
 // ------------------------------------------------------------------------------------------------
-// Fast kernel: one persistent CTA per simulation.
+// Shared-memory access by 32-bit shared-window address (no generic-address arithmetic in the hot loops).
 // ------------------------------------------------------------------------------------------------
-#ifndef FIRE_LB_THREADS      // tuning builds: -DFIRE_LB_THREADS=256 -DFIRE_LB_CTAS=6 caps the registers for that geometry
-#define FIRE_LB_THREADS 1024
-#define FIRE_LB_CTAS 1
+__device__ __forceinline__ void sts64(uint32_t addr, uint32_t a, uint32_t b)
+{
+    asm volatile("st.shared.v2.u32 [%0], {%1, %2};" :: "r"(addr), "r"(a), "r"(b) : "memory");
+}
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t a)
+{
+    asm volatile("st.shared.u32 [%0], %1;" :: "r"(addr), "r"(a) : "memory");
+}
+__device__ __forceinline__ uint2 lds64(uint32_t addr)
+{
+    uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory"); return v;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr)
+{
+    uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
+}
+
+// List / queue slots beyond the shared-memory part (rare: only very long fronts get here).
+__device__ __noinline__ void spill_put_q(uint32_t qs_addr, uint2* Qg, uint32_t capQ_s, uint32_t q, uint32_t item, uint32_t T)
+{
+    if (q < capQ_s) sts64(qs_addr + 8u * q, item, T); else __stcg(Qg + (q - capQ_s), make_uint2(item, T));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Per-step context of one simulation (everything the two pass functions need; all warp-invariant).
+// ------------------------------------------------------------------------------------------------
+struct step_ctx {
+    // lattice / tables
+    uint32_t W, Tw, Th;
+    const uint64_t* sus;          // susceptible plane of this simulation, tile layout
+    uint32_t* sus32;              // the same, as 8 x 4-cell half tiles (atomics)
+    const uint4* thr4;            // threshold sectors of this simulation's parameter vector, 2 x uint4 per source cell
+    // lists
+    uint32_t qs_addr, ac_addr, an_addr;   // shared-window addresses: trial queue, current frontier, next frontier
+    uint32_t capQ_s, capA_s, capA;
+    uint2* Qg; const uint32_t* Ac_g; uint32_t* An_g;
+    unsigned int* cntQ; unsigned int* cntA_next; unsigned int* over;
+    uint32_t nA, nQ;
+    uint32_t lane, lt;
+};
+
+// Phase 1 for K units of 32 burning cells (units u0, u0 + ustride, ...; all of them exist: u * 32 < nA).
+// Lanes past the end of the list re-read the last entry and contribute nothing.
+template <int K>
+__device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, uint32_t ustride)
+{
+    uint32_t e[K], win[K];
+    uint64_t tc[K], th[K], tv[K], td[K];
+    uint4 Ta[K], Tb[K];
+    bool live[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        uint32_t i = (u0 + (uint32_t)k * ustride) * 32u + c.lane;
+        live[k] = i < c.nA;
+        i = live[k] ? i : c.nA - 1u;
+        e[k] = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.Ac_g + (i - c.capA_s));
+        const uint32_t x = e[k] & 0xFFFFu, y = e[k] >> 16;
+        const uint32_t tx0 = x >> 3, ty0 = y >> 3, bx = x & 7u, by = y & 7u;
+        const uint32_t tidx = ty0 * c.Tw + tx0;
+        const int hoff = (bx == 0u && tx0 > 0u) ? -1 : ((bx == 7u && tx0 + 1u < c.Tw) ? 1 : 0);
+        const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
+        const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
+        tc[k] = ldcg_u64(c.sus + tidx);
+        Ta[k] = ldg_thr(sp);
+        Tb[k] = ldg_thr(sp + 1);
+        th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
+        if (hoff) th[k] = ldcg_u64(c.sus + (tidx + hoff));
+        if (voff) tv[k] = ldcg_u64(c.sus + (tidx + voff));
+        if (hoff && voff) td[k] = ldcg_u64(c.sus + (tidx + hoff + voff));
+    }
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const uint32_t bx = e[k] & 7u, by = (e[k] >> 16) & 7u;
+        // rows y-1, y, y+1 of the cell's tile column (w3c) and of the horizontally adjacent one (w3h), one per byte
+        const uint32_t selr = ((by + 7u) & 7u) | (by << 4) | (((by + 1u) & 7u) << 8);
+        uint32_t w3c = __byte_perm((uint32_t)tc[k], (uint32_t)(tc[k] >> 32), selr) & 0xFFFFFFu;
+        uint32_t w3h = __byte_perm((uint32_t)th[k], (uint32_t)(th[k] >> 32), selr) & 0xFFFFFFu;
+        // row y-1 is row 7 of the tile above when by == 0, row y+1 is row 0 of the tile below when by == 7
+        const uint32_t vc = (by == 0u) ? (uint32_t)(tv[k] >> 56) : (((uint32_t)tv[k] & 0xFFu) << 16);
+        const uint32_t vh = (by == 0u) ? (uint32_t)(td[k] >> 56) : (((uint32_t)td[k] & 0xFFu) << 16);
+        const uint32_t keep = (by == 0u) ? 0xFFFF00u : ((by == 7u) ? 0x00FFFFu : 0xFFFFFFu);
+        w3c = (w3c & keep) | vc;                                     // tv = td = 0 unless by is 0 or 7
+        w3h = (w3h & keep) | vh;
+        // per byte: bit 0 = (x-1), bit 1 = x, bit 2 = (x+1)
+        const uint32_t tcen = (w3c << 1) >> bx;
+        const uint32_t mC = (bx == 0u) ? 0x060606u : ((bx == 7u) ? 0x030303u : 0x070707u);
+        const uint32_t hb = (bx == 0u) ? ((w3h >> 7) & 0x010101u) : ((w3h << 2) & 0x040404u);
+        win[k] = live[k] ? ((tcen & mC) | hb) : 0u;
+        cnt += __popc(win[k]);
+    }
+    uint32_t incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (c.lane >= (uint32_t)o) incl += v;
+    }
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    if (total == 0) return 0u;
+    uint32_t qbase = 0;
+    if (c.lane == 31) qbase = atomicAdd(c.cntQ, total);
+    qbase = __shfl_sync(0xFFFFFFFFu, qbase, 31);
+    uint32_t pos = qbase + incl - cnt;
+    if (qbase + total <= c.capQ_s) {                                  // warp-uniform: the whole batch fits in shared memory
+#define FIRE_EMIT(bit, d, Tv) \
+        if (w & (1u << (bit))) sts64(qa + 8u * __popc(w & ((1u << (bit)) - 1u)), base + item_delta(d), (Tv));
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint32_t w = win[k];
+            const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
+            const uint32_t qa = c.qs_addr + 8u * pos;
+            FIRE_EMIT(0, 7, Tb[k].w)  FIRE_EMIT(1, 0, Ta[k].x)  FIRE_EMIT(2, 1, Ta[k].y)
+            FIRE_EMIT(8, 6, Tb[k].z)  FIRE_EMIT(10, 2, Ta[k].z)
+            FIRE_EMIT(16, 5, Tb[k].y) FIRE_EMIT(17, 4, Tb[k].x) FIRE_EMIT(18, 3, Ta[k].w)
+            pos += __popc(w);
+        }
+#undef FIRE_EMIT
+    } else {
+#define FIRE_EMIT(bit, d, Tv) \
+        if (w & (1u << (bit))) spill_put_q(c.qs_addr, c.Qg, c.capQ_s, pos + __popc(w & ((1u << (bit)) - 1u)), base + item_delta(d), (Tv));
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const uint32_t w = win[k];
+            const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
+            FIRE_EMIT(0, 7, Tb[k].w)  FIRE_EMIT(1, 0, Ta[k].x)  FIRE_EMIT(2, 1, Ta[k].y)
+            FIRE_EMIT(8, 6, Tb[k].z)  FIRE_EMIT(10, 2, Ta[k].z)
+            FIRE_EMIT(16, 5, Tb[k].y) FIRE_EMIT(17, 4, Tb[k].x) FIRE_EMIT(18, 3, Ta[k].w)
+            pos += __popc(w);
+        }
+#undef FIRE_EMIT
+    }
+    return cnt;
+}
+
+// Philox keys and the per-step constants of rounds 0 and 1 (C-1; rounds 0 and 1 see (c1, c2) = (t, sim)).
+struct philox_step {
+    uint32_t rk0[10], rk1[10];   // round keys (rk0[0], rk0[1], rk1[1] are folded into the constants below)
+    uint32_t x1, y1, a1l;
+};
+
+// Phase 2 for K units of 32 trials (units u0, u0 + ustride, ...; all of them exist: u * 32 < nQ).
+// Stages, so that each long latency is waited for once per pass: queue reads -> Philox -> atomics -> compaction.
+template <int K>
+__device__ __forceinline__ void trials_pass(const step_ctx& c, const philox_step& ph, uint32_t u0, uint32_t ustride)
+{
+    uint32_t item[K], T[K];
+    const bool q_shared = (u0 + (uint32_t)(K - 1) * ustride + 1u) * 32u <= c.capQ_s;      // warp-uniform
+#pragma unroll
+    for (int u = 0; u < K; ++u) {
+        uint32_t j = (u0 + (uint32_t)u * ustride) * 32u + c.lane;
+        const bool live = j < c.nQ;
+        j = live ? j : c.nQ - 1u;
+        const uint2 it = (q_shared || j < c.capQ_s) ? lds64(c.qs_addr + 8u * j) : __ldcg(c.Qg + (j - c.capQ_s));
+        item[u] = it.x;
+        T[u] = live ? it.y : 0u;                                   // T = 0 never succeeds
+    }
+    bool succ[K];
+    uint32_t widx[K], bit[K], old[K];
+#pragma unroll
+    for (int u = 0; u < K; ++u) {
+        const uint32_t ty = item[u] >> 16, tx = (item[u] >> 3) & 0x1FFFu, d = item[u] & 7u;
+        const uint32_t cell = ty * c.W + tx;
+        bit[u] = ((ty & 3u) << 3) | (tx & 7u);
+        widx[u] = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
+        // round 0: (cell, t, sim, d >> 2) -> (r0c0, bl, hi(cell * M0) ^ (d >> 2) ^ k1, lo(cell * M0))
+        uint32_t c3 = cell * kM0;
+        uint32_t c2 = __umulhi(cell, kM0) ^ (d >> 2) ^ ph.rk1[0];
+        // round 1: a = r0c0 * M0 (per step), b = c2 * M1
+        uint32_t c0 = __umulhi(c2, kM1) ^ ph.x1;
+        uint32_t c1 = c2 * kM1;
+        c2 = ph.y1 ^ c3;
+        c3 = ph.a1l;
+#pragma unroll
+        for (int r = 2; r < 10; ++r) {
+            const uint64_t a = (uint64_t)c0 * kM0;
+            const uint64_t b = (uint64_t)c2 * kM1;
+            const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ ph.rk0[r];
+            const uint32_t n2 = (uint32_t)(a >> 32) ^ c3 ^ ph.rk1[r];
+            c1 = (uint32_t)b; c3 = (uint32_t)a; c0 = n0; c2 = n2;
+        }
+        const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
+        const uint32_t rnd = (d & 2u) ? hi : lo;
+        succ[u] = fire_trial(rnd, T[u]);
+    }
+#pragma unroll
+    for (int u = 0; u < K; ++u) {
+        old[u] = 0u;
+        if (succ[u]) old[u] = atomicAnd(c.sus32 + widx[u], ~(1u << bit[u]));
+#ifdef FIRE_PREFETCH_THR
+        if (succ[u]) asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)((((item[u] >> 16) * c.W + ((item[u] >> 3) & 0x1FFFu))) * 2u)));
 #endif
-__global__ void __launch_bounds__(FIRE_LB_THREADS, FIRE_LB_CTAS)
+    }
+    uint32_t fresh_mask[K];
+    uint32_t n_fresh = 0;
+#pragma unroll
+    for (int u = 0; u < K; ++u) {
+        fresh_mask[u] = __ballot_sync(0xFFFFFFFFu, (old[u] >> bit[u]) & 1u);     // old = 0 unless the trial succeeded
+        n_fresh += __popc(fresh_mask[u]);
+    }
+    if (n_fresh == 0) return;                                      // warp-uniform
+    uint32_t abase = 0;
+    if (c.lane == 0) abase = atomicAdd(c.cntA_next, n_fresh);
+    abase = __shfl_sync(0xFFFFFFFFu, abase, 0);
+    if (abase + n_fresh <= c.capA_s) {                             // warp-uniform: all new cells go to shared memory
+#pragma unroll
+        for (int u = 0; u < K; ++u) {
+            const uint32_t en = (item[u] & 0xFFFF0000u) | ((item[u] >> 3) & 0x1FFFu);
+            const uint32_t a = c.an_addr + 4u * (abase + __popc(fresh_mask[u] & c.lt));
+            if (fresh_mask[u] & (1u << c.lane)) sts32(a, en);
+            abase += __popc(fresh_mask[u]);
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < K; ++u) {
+            if (fresh_mask[u] & (1u << c.lane)) {
+                const uint32_t pos = abase + __popc(fresh_mask[u] & c.lt);
+                const uint32_t en = (item[u] & 0xFFFF0000u) | ((item[u] >> 3) & 0x1FFFu);
+                if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, en);
+                else if (pos < c.capA) __stcg(c.An_g + (pos - c.capA_s), en);
+                else *c.over = 1u;
+            }
+            abase += __popc(fresh_mask[u]);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fast kernel: one persistent CTA per simulation.
+// Instantiated for a few (threads per CTA, CTAs per SM) bounds: the bound sets the register budget.
+// kCellsInFlight / kTrialsInFlight: units of 32 burning cells (phase 1) / 32 trials (phase 2) a warp has in flight.
+// ------------------------------------------------------------------------------------------------
+template <int kMaxThreads, int kMinCtas, int kCellsInFlight, int kTrialsInFlight>
+__global__ void __launch_bounds__(kMaxThreads, kMinCtas)
 fire_propagate_kernel(const prop_params prm)
 {
     extern __shared__ __align__(16) uint32_t smem[];
-    const uint32_t capA_s = prm.capA_s, capQ_s = prm.capQ_s;
-    uint2* const Qs = reinterpret_cast<uint2*>(smem);
-    uint32_t* const As0 = smem + 2 * (size_t)capQ_s;
-    uint32_t* const As1 = As0 + capA_s;
-    const size_t spill_per_cta = (size_t)2 * (prm.capQ - capQ_s) + (size_t)2 * (prm.capA - capA_s);
-    uint2* const Qg = reinterpret_cast<uint2*>(prm.spill + (size_t)blockIdx.x * spill_per_cta);
-    uint32_t* const Ag0 = prm.spill + (size_t)blockIdx.x * spill_per_cta + (size_t)2 * (prm.capQ - capQ_s);
-    uint32_t* const Ag1 = Ag0 + (prm.capA - capA_s);
+    // shared layout: trial queue (capQ_s x 8 B), frontier list 0, frontier list 1 (capA_s x 4 B each)
+    uint32_t qs_addr = (uint32_t)__cvta_generic_to_shared(smem);
+    asm volatile("" : "+r"(qs_addr));            // keep it in a register: ptxas would otherwise rebuild the window address at every use
+    const uint32_t as_addr0 = qs_addr + 8u * prm.capQ_s, as_addr1 = as_addr0 + 4u * prm.capA_s;
+    const size_t spill_per_cta = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);
+    uint32_t* const Ag0 = prm.spill + (size_t)blockIdx.x * spill_per_cta + (size_t)2 * (prm.capQ - prm.capQ_s);
+    uint32_t* const Ag1 = Ag0 + (prm.capA - prm.capA_s);
 
     __shared__ unsigned int s_sim, s_cntA[2], s_cntQ[2], s_over;
     __shared__ unsigned long long s_trials;
 
-    const int tid = threadIdx.x, lane = tid & 31, nthr = blockDim.x;
-    const int W = prm.W, H = prm.H, Tw = prm.Tw, Th = prm.Th;
-    const uint32_t lt = lanemask_lt();
+    const int tid = threadIdx.x;
+    const uint32_t warp = (uint32_t)tid >> 5, nwarps = blockDim.x >> 5;
+
+    step_ctx c;
+    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th;
+    c.qs_addr = qs_addr; c.capQ_s = prm.capQ_s; c.capA_s = prm.capA_s; c.capA = prm.capA;
+    c.Qg = reinterpret_cast<uint2*>(prm.spill + (size_t)blockIdx.x * spill_per_cta);
+    c.over = &s_over;
+    c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
 
     for (;;) {
         __syncthreads();                       // the previous simulation's last reads of s_* are done
@@ -122,17 +353,22 @@ fire_propagate_kernel(const prop_params prm)
         __syncthreads();
         const uint32_t s = s_sim;
         if (s == 0xFFFFFFFFu) break;
+#ifdef FIRE_TRACE
+        unsigned long long trace_t0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t0));
+#endif
 
         const int p = prm.sim_param[s];
         const int ix = prm.ignitions[2 * s], iy = prm.ignitions[2 * s + 1];
         const uint64_t seed = prm.seeds[s];
         const uint32_t sim = prm.sim_ids ? (uint32_t)prm.sim_ids[s] : s;
-        uint64_t* const sus = prm.tiles + (size_t)s * Tw * Th;
-        uint32_t* const sus32 = reinterpret_cast<uint32_t*>(sus);
-        bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < W && iy >= 0 && iy < H;     // R-12
+        c.sus = prm.tiles + (size_t)s * c.Tw * c.Th;
+        c.sus32 = reinterpret_cast<uint32_t*>(prm.tiles + (size_t)s * c.Tw * c.Th);
+        bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
         if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
-        const uint32_t* const thr = prm.thr + (valid ? (size_t)p * W * H * 8 : 0);
-        const uint32_t key_lo = (uint32_t)seed, key_hi = (uint32_t)(seed >> 32);
+        c.thr4 = reinterpret_cast<const uint4*>(prm.thr + (valid ? (size_t)p * c.W * prm.H * 8 : 0));
+        // the key is the same in every lane: a warp reduction leaves it in a UNIFORM register, and so are the round keys
+        // derived from it (they then cost no per-thread registers)
+        const uint32_t key_lo = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)seed), key_hi = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)(seed >> 32));
         // Philox round 0 multiplies the counter word `sim` by M1: the same product for every trial of the simulation
         const uint32_t bh = __umulhi(sim, kM1), bl = sim * kM1;
 
@@ -141,205 +377,63 @@ fire_propagate_kernel(const prop_params prm)
             s_over = 0u; s_trials = 0ull;
             if (valid) {
                 const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
-                if (capA_s > 0) As0[0] = e0; else Ag0[0] = e0;
-                atomicAnd(sus32 + (((size_t)(iy >> 3) * Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
+                if (prm.capA_s > 0) sts32(as_addr0, e0); else Ag0[0] = e0;
+                atomicAnd(c.sus32 + (((size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
         }
         __syncthreads();
 
         uint32_t t = 0, my_trials = 0;
-        uint32_t nA = valid ? 1u : 0u;
+        c.nA = valid ? 1u : 0u;
         bool over = false;
-        while (nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
-            const int par = t & 1;
-            const uint32_t* const Ac_s = par ? As1 : As0;  const uint32_t* const Ac_g = par ? Ag1 : Ag0;
-            uint32_t* const An_s = par ? As0 : As1;        uint32_t* const An_g = par ? Ag0 : Ag1;
+        while (c.nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
+            const uint32_t par = t & 1u;
+            c.ac_addr = par ? as_addr1 : as_addr0; c.an_addr = par ? as_addr0 : as_addr1;
+            c.Ac_g = par ? Ag1 : Ag0; c.An_g = par ? Ag0 : Ag1;
+            c.cntQ = &s_cntQ[par]; c.cntA_next = &s_cntA[par ^ 1u];
 
             // ---- phase 1: susceptible neighbours of the burning cells and their thresholds -> trial queue.
-            // kCellsInFlight burning cells per lane; all their loads are issued before any is used.
-            for (uint32_t i0 = (uint32_t)(tid & ~31) * kCellsInFlight; i0 < nA; i0 += (uint32_t)nthr * kCellsInFlight) {
-                uint32_t e[kCellsInFlight], win[kCellsInFlight];
-                uint64_t tc[kCellsInFlight], th[kCellsInFlight], tv[kCellsInFlight], td[kCellsInFlight];
-                uint4 Ta[kCellsInFlight], Tb[kCellsInFlight];
-#pragma unroll
-                for (int k = 0; k < kCellsInFlight; ++k) {
-                    const uint32_t i = i0 + 32u * k + lane;
-                    e[k] = 0xFFFFFFFFu; tc[k] = 0ull; th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
-                    Ta[k] = make_uint4(0u, 0u, 0u, 0u); Tb[k] = make_uint4(0u, 0u, 0u, 0u);
-                    if (i < nA) {
-                        e[k] = (i < capA_s) ? Ac_s[i] : __ldcg(Ac_g + (i - capA_s));
-                        const int x = (int)(e[k] & 0xFFFFu), y = (int)(e[k] >> 16);
-                        const int tx0 = x >> 3, ty0 = y >> 3, bx = x & 7, by = y & 7;
-                        const int hoff = (bx == 0 && tx0 > 0) ? -1 : ((bx == 7 && tx0 + 1 < Tw) ? 1 : 0);
-                        const int voff = (by == 0 && ty0 > 0) ? -Tw : ((by == 7 && ty0 + 1 < Th) ? Tw : 0);
-                        const uint64_t* const tp = sus + ((size_t)ty0 * Tw + tx0);
-                        const uint4* const sp = reinterpret_cast<const uint4*>(thr + ((size_t)y * W + x) * 8);
-                        tc[k] = ldcg_u64(tp);
-                        Ta[k] = ldg_thr(sp);
-                        Tb[k] = ldg_thr(sp + 1);
-                        if (hoff) th[k] = ldcg_u64(tp + hoff);
-                        if (voff) tv[k] = ldcg_u64(tp + voff);
-                        if (hoff && voff) td[k] = ldcg_u64(tp + hoff + voff);
-                    }
-                }
-                uint32_t cnt = 0;
-#pragma unroll
-                for (int k = 0; k < kCellsInFlight; ++k) {
-                    win[k] = 0u;
-                    if (e[k] != 0xFFFFFFFFu) {
-                        const uint32_t bx = e[k] & 7u, by = (e[k] >> 16) & 7u;
-                        // rows y-1, y, y+1 of the cell's tile column (w3c) and of the horizontally adjacent one (w3h), one per byte
-                        const uint32_t selr = ((by + 7u) & 7u) | (by << 4) | (((by + 1u) & 7u) << 8);
-                        uint32_t w3c = __byte_perm((uint32_t)tc[k], (uint32_t)(tc[k] >> 32), selr) & 0xFFFFFFu;
-                        uint32_t w3h = __byte_perm((uint32_t)th[k], (uint32_t)(th[k] >> 32), selr) & 0xFFFFFFu;
-                        if (by == 0u) {            // row y-1 is row 7 of the tile above (or does not exist)
-                            w3c = (w3c & 0xFFFF00u) | (uint32_t)(tv[k] >> 56);
-                            w3h = (w3h & 0xFFFF00u) | (uint32_t)(td[k] >> 56);
-                        } else if (by == 7u) {     // row y+1 is row 0 of the tile below
-                            w3c = (w3c & 0x00FFFFu) | (((uint32_t)tv[k] & 0xFFu) << 16);
-                            w3h = (w3h & 0x00FFFFu) | (((uint32_t)td[k] & 0xFFu) << 16);
-                        }
-                        // per byte: bit 0 = (x-1), bit 1 = x, bit 2 = (x+1)
-                        const uint32_t tcen = (w3c << 1) >> bx;
-                        const uint32_t mC = (bx == 0u) ? 0x060606u : ((bx == 7u) ? 0x030303u : 0x070707u);
-                        const uint32_t hb = (bx == 0u) ? ((w3h >> 7) & 0x010101u) : ((w3h << 2) & 0x040404u);
-                        win[k] = (tcen & mC) | hb;
-                    }
-                    cnt += __popc(win[k]);
-                }
-                uint32_t incl = cnt;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-                    if (lane >= o) incl += v;
-                }
-                const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-                if (total == 0) continue;
-                uint32_t qbase = 0;
-                if (lane == 31) qbase = atomicAdd(&s_cntQ[par], total);
-                qbase = __shfl_sync(0xFFFFFFFFu, qbase, 31);
-                uint32_t pos = qbase + incl - cnt;
-                my_trials += cnt;
-                const bool in_shared = qbase + total <= capQ_s;           // warp-uniform: the whole batch fits in shared memory
-#define FIRE_EMIT(bit, d, Tv)                                                                          \
-                    if (w & (1u << (bit))) {                                                           \
-                        const uint32_t q = pos + __popc(w & ((1u << (bit)) - 1u));                     \
-                        const uint2 it = make_uint2(base + item_delta(d), (Tv));                       \
-                        if (in_shared || q < capQ_s) Qs[q] = it; else __stcg(Qg + (q - capQ_s), it);   \
-                    }
-#pragma unroll
-                for (int k = 0; k < kCellsInFlight; ++k) {
-                    const uint32_t w = win[k];
-                    const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
-                    FIRE_EMIT(0, 7, Tb[k].w)  FIRE_EMIT(1, 0, Ta[k].x)  FIRE_EMIT(2, 1, Ta[k].y)
-                    FIRE_EMIT(8, 6, Tb[k].z)  FIRE_EMIT(10, 2, Ta[k].z)
-                    FIRE_EMIT(16, 5, Tb[k].y) FIRE_EMIT(17, 4, Tb[k].x) FIRE_EMIT(18, 3, Ta[k].w)
-                    pos += __popc(w);
-                }
-#undef FIRE_EMIT
+            // Units of 32 cells are dealt round-robin to the warps: full passes of kCellsInFlight units, then single units.
+            {
+                const uint32_t nU = (c.nA + 31u) >> 5;
+                uint32_t u = warp;
+                if (kCellsInFlight > 1)
+                    for (; u + (uint32_t)(kCellsInFlight - 1) * nwarps < nU; u += nwarps * kCellsInFlight)
+                        my_trials += cells_pass<kCellsInFlight>(c, u, nwarps);
+                for (; u < nU; u += nwarps) my_trials += cells_pass<1>(c, u, nwarps);
             }
             __syncthreads();
-            const uint32_t nQ = s_cntQ[par];
-            if (tid == 0) { s_cntA[par] = 0u; s_cntQ[par ^ 1] = 0u; }     // next step's counters; nobody reads them now
+            c.nQ = s_cntQ[par];
+            if (tid == 0) { s_cntA[par] = 0u; s_cntQ[par ^ 1u] = 0u; }    // next step's counters; nobody reads them now
 
-            // ---- phase 2: one Bernoulli trial per lane-slot, kTrialsInFlight per lane, in stages so that each
-            // long latency is waited for once per batch: queue reads -> Philox -> atomics -> compaction.
-            // Philox4x32-10(counter = (c, t, sim, d >> 2), key = seed), word d & 3 (C-1).  Round keys are
-            // rebuilt here once per step (they are dead during phase 1) and made opaque so that they stay in registers.
-            uint32_t rk0[10], rk1[10];
+            // ---- phase 2: one Bernoulli trial per lane-slot.  Philox4x32-10(counter = (cell, t, sim, d >> 2), key = seed),
+            // word d & 3 (C-1).  Round keys are rebuilt once per step (they are dead during phase 1) and made
+            // opaque so that they stay in registers.
+            {
+                philox_step ph;
 #pragma unroll
-            for (int r = 0; r < 10; ++r) {
-                rk0[r] = key_lo + (uint32_t)r * kW0;
-                rk1[r] = key_hi + (uint32_t)r * kW1;
-                asm volatile("" : "+r"(rk0[r]), "+r"(rk1[r]));
-            }
-            // rounds 0 and 1 see (c1, c2) = (t, sim): everything that does not depend on the cell is per-step
-            const uint32_t r0c0 = bh ^ t ^ rk0[0];                      // c0 after round 0
-            const uint32_t a1h = __umulhi(r0c0, kM0), a1l = r0c0 * kM0; // round 1: c0 * M0
-            const uint32_t x1 = bl ^ rk0[1], y1 = a1h ^ rk1[1];
-            for (uint32_t j0 = (uint32_t)(tid & ~31) * kTrialsInFlight; j0 < nQ; j0 += (uint32_t)nthr * kTrialsInFlight) {
-                uint32_t item[kTrialsInFlight], T[kTrialsInFlight], old[kTrialsInFlight];
-                const bool q_shared = j0 + 32u * kTrialsInFlight <= capQ_s;     // warp-uniform
-#pragma unroll
-                for (int u = 0; u < kTrialsInFlight; ++u) {
-                    const uint32_t j = j0 + 32u * u + lane;
-                    item[u] = 0xFFFFFFFFu;
-                    T[u] = 0u;
-                    if (j < nQ) {
-                        const uint2 it = (q_shared || j < capQ_s) ? Qs[j] : __ldcg(Qg + (j - capQ_s));
-                        item[u] = it.x; T[u] = it.y;
-                    }
-                }
-                bool succ[kTrialsInFlight];
-#pragma unroll
-                for (int u = 0; u < kTrialsInFlight; ++u) {
-                    succ[u] = false;
-                    if (j0 + 32u * u < nQ) {                               // warp-uniform
-                        const uint32_t ty = item[u] >> 16, tx = (item[u] >> 3) & 0x1FFFu, d = item[u] & 7u;
-                        const uint32_t cell = ty * (uint32_t)W + tx;
-                        // round 0: (cell, t, sim, d >> 2) -> (r0c0, bl, hi(cell * M0) ^ (d >> 2) ^ k1, lo(cell * M0))
-                        uint32_t c3 = cell * kM0;
-                        uint32_t c2 = __umulhi(cell, kM0) ^ (d >> 2) ^ rk1[0];
-                        // round 1: a = r0c0 * M0 (per step), b = c2 * M1
-                        uint32_t c0 = __umulhi(c2, kM1) ^ x1;
-                        uint32_t c1 = c2 * kM1;
-                        c2 = y1 ^ c3;
-                        c3 = a1l;
-#pragma unroll
-                        for (int r = 2; r < 10; ++r) {
-                            const uint64_t a = (uint64_t)c0 * kM0;
-                            const uint64_t b = (uint64_t)c2 * kM1;
-                            const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ rk0[r];
-                            const uint32_t n2 = (uint32_t)(a >> 32) ^ c3 ^ rk1[r];
-                            c1 = (uint32_t)b; c3 = (uint32_t)a; c0 = n0; c2 = n2;
-                        }
-                        const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
-                        const uint32_t rnd = (d & 2u) ? hi : lo;
-                        succ[u] = item[u] != 0xFFFFFFFFu && fire_trial(rnd, T[u]);
-                    }
-                }
-#pragma unroll
-                for (int u = 0; u < kTrialsInFlight; ++u) {
-                    old[u] = 0u;
-                    if (succ[u]) {
-                        const uint32_t ty = item[u] >> 16, tx = (item[u] >> 3) & 0x1FFFu;
-                        const uint32_t widx = (((ty >> 3) * (uint32_t)Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
-                        old[u] = atomicAnd(sus32 + widx, ~(1u << (((ty & 3u) << 3) | (tx & 7u))));
-#ifdef FIRE_PREFETCH_THR
-                        asm volatile("prefetch.global.L2 [%0];" :: "l"(thr + ((size_t)(ty * (uint32_t)W + tx)) * 8));
+                for (int r = 0; r < 10; ++r) {
+                    ph.rk0[r] = key_lo + (uint32_t)r * kW0;
+                    ph.rk1[r] = key_hi + (uint32_t)r * kW1;
+#ifdef FIRE_KEYS_IN_VECTOR_REGS
+                    asm volatile("" : "+r"(ph.rk0[r]), "+r"(ph.rk1[r]));
 #endif
-                    }
                 }
-                uint32_t fresh_mask[kTrialsInFlight];
-                uint32_t n_fresh = 0;
-#pragma unroll
-                for (int u = 0; u < kTrialsInFlight; ++u) {
-                    const uint32_t bit = (((item[u] >> 16) & 3u) << 3) | ((item[u] >> 3) & 7u);
-                    const bool fresh = succ[u] && ((old[u] >> bit) & 1u);
-                    fresh_mask[u] = __ballot_sync(0xFFFFFFFFu, fresh);
-                    n_fresh += __popc(fresh_mask[u]);
-                }
-                if (n_fresh == 0) continue;                                // warp-uniform
-                uint32_t abase = 0;
-                if (lane == 0) abase = atomicAdd(&s_cntA[par ^ 1], n_fresh);
-                abase = __shfl_sync(0xFFFFFFFFu, abase, 0);
-                const bool a_shared = abase + n_fresh <= capA_s;           // warp-uniform
-#pragma unroll
-                for (int u = 0; u < kTrialsInFlight; ++u) {
-                    if (fresh_mask[u] & (1u << lane)) {
-                        const uint32_t pos = abase + __popc(fresh_mask[u] & lt);
-                        const uint32_t en = (item[u] & 0xFFFF0000u) | ((item[u] >> 3) & 0x1FFFu);
-                        if (a_shared || pos < capA_s) An_s[pos] = en;
-                        else if (pos < prm.capA) __stcg(An_g + (pos - capA_s), en);
-                        else s_over = 1u;
-                    }
-                    abase += __popc(fresh_mask[u]);
-                }
+                const uint32_t r0c0 = bh ^ t ^ ph.rk0[0];                          // c0 after round 0
+                ph.a1l = r0c0 * kM0;                                               // round 1: c0 * M0
+                ph.x1 = bl ^ ph.rk0[1];
+                ph.y1 = __umulhi(r0c0, kM0) ^ ph.rk1[1];
+                const uint32_t nU = (c.nQ + 31u) >> 5;
+                uint32_t u = warp;
+                if (kTrialsInFlight > 1)
+                    for (; u + (uint32_t)(kTrialsInFlight - 1) * nwarps < nU; u += nwarps * kTrialsInFlight)
+                        trials_pass<kTrialsInFlight>(c, ph, u, nwarps);
+                for (; u < nU; u += nwarps) trials_pass<1>(c, ph, u, nwarps);
             }
             __syncthreads();
             ++t;
             if (s_over) { over = true; break; }       // written in phase 2 only, read after its closing barrier
-            nA = s_cntA[par ^ 1];
+            c.nA = s_cntA[par ^ 1u];
         }
 
         // ---- end of the simulation
@@ -351,6 +445,10 @@ fire_propagate_kernel(const prop_params prm)
             } else {
                 if (prm.out_steps) prm.out_steps[s] = t;
                 if (prm.out_trials) prm.out_trials[s] = s_trials;
+#ifdef FIRE_TRACE   // diagnostic build only: out_trials = (start us << 32) | duration us of this simulation, for schedule plots
+                unsigned long long trace_t1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t1));
+                if (prm.out_trials) prm.out_trials[s] = (((trace_t0 / 1000ull) & 0xFFFFFFFFull) << 32) | (((trace_t1 - trace_t0) / 1000ull) & 0xFFFFFFFFull);
+#endif
             }
         }
     }
@@ -584,6 +682,14 @@ extern "C" int fire_set_list_capacity(fire_landscape* L, int32_t shared_entries,
     return FIRE_OK;
 }
 
+extern "C" int fire_set_schedule(fire_landscape* L, int32_t mode)
+{
+    if (L == nullptr || mode < 0) return FIRE_EINVAL;
+    L->schedule = mode & 1;
+    L->kernel_variant = mode >> 4;       // tuning builds: bits 4.. select an instantiation of the kernel
+    return FIRE_OK;
+}
+
 extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, const int32_t* sim_param,
                                    const uint64_t* seeds, const int32_t* sim_ids, int32_t S, uint32_t max_steps,
                                    uint32_t* out_burned, uint32_t* out_steps, uint64_t* out_trials, void* stream)
@@ -596,8 +702,17 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     cudaStream_t st = (cudaStream_t)stream;
 
     // ---- geometry and list capacities
-    const int threads = L->threads_per_cta ? L->threads_per_cta : 256;
-    const int per_sm = L->ctas_per_sm ? L->ctas_per_sm : 4;
+    // default: 1024 threads per SM, as 4 CTAs of 256 threads when there are enough simulations to fill them,
+    // else fewer and wider CTAs so that a small batch of large fires still uses whole SMs
+    int threads = L->threads_per_cta, per_sm = L->ctas_per_sm;
+    if (threads == 0 && per_sm == 0) {
+        if ((long long)S >= 4ll * L->num_sms) { threads = 256; per_sm = 4; }
+        else if ((long long)S >= 2ll * L->num_sms) { threads = 512; per_sm = 2; }
+        else { threads = 1024; per_sm = 1; }
+    } else {
+        if (threads == 0) threads = 256;
+        if (per_sm == 0) per_sm = (1024 / threads) > 0 ? (1024 / threads) : 1;
+    }
     const int grid = (int)((long long)S < (long long)L->num_sms * per_sm ? S : L->num_sms * per_sm);
     prop_params prm;
     uint32_t capA_s = L->list_shared ? (uint32_t)L->list_shared : 1536u;
@@ -613,7 +728,8 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     if (capA_s > capA) capA_s = capA;
     prm.capA_s = capA_s; prm.capA = capA;
     prm.capQ = 8u * capA;
-    prm.capQ_s = 2u * capA_s < prm.capQ ? 2u * capA_s : prm.capQ;
+    prm.capQ_s = 2u * capA_s;                                  // default: 1536-cell lists + 3072-trial queue = 36 KiB per CTA
+    if (prm.capQ_s > prm.capQ) prm.capQ_s = prm.capQ;
     const size_t smem = ((size_t)2 * prm.capA_s + (size_t)2 * prm.capQ_s) * sizeof(uint32_t);
     if (smem > 200 * 1024) return FIRE_EINVAL;
 
@@ -662,7 +778,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
 
     // ---- launch order: largest expected fires first (only matters when there are more simulations than resident CTAs)
     prm.order = nullptr;
-    if (S > grid && L->param_mean != nullptr) {
+    if (S > grid && L->param_mean != nullptr && L->schedule == 0) {
         fire_order_kernel<<<1, 1024, 0, st>>>(sim_param, L->param_mean, S, L->P, 1.0f / ((float)L->cells * 8.0f), L->order);
         FIRE_CUDA_TRY(L, cudaGetLastError());
         L->launches += 1;
@@ -679,11 +795,22 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
     FIRE_CUDA_TRY(L, cudaMemsetAsync(L->work_counter, 0, 2 * sizeof(unsigned int), st));
+    void (*kernel)(const prop_params) = fire_propagate_kernel<1024, 1, 2, 4>;
+    const int variant = L->kernel_variant;
+    if (threads <= 256 && per_sm >= 8)
+        kernel = variant == 1 ? fire_propagate_kernel<256, 8, 1, 1> : (variant == 2 ? fire_propagate_kernel<256, 8, 1, 4> : fire_propagate_kernel<256, 8, 1, 2>);
+    else if (threads <= 256 && per_sm >= 6)
+        kernel = variant == 1 ? fire_propagate_kernel<256, 6, 1, 2> : (variant == 2 ? fire_propagate_kernel<256, 6, 1, 4> : fire_propagate_kernel<256, 6, 2, 4>);
+    else if (threads <= 256 && per_sm == 5)
+        kernel = variant == 1 ? fire_propagate_kernel<256, 5, 1, 2> : (variant == 2 ? fire_propagate_kernel<256, 5, 1, 4> : fire_propagate_kernel<256, 5, 2, 4>);
+    else if (threads <= 256)
+        kernel = variant == 2 ? fire_propagate_kernel<256, 4, 1, 4> : fire_propagate_kernel<256, 4, 2, 4>;
+    else if (threads <= 512) kernel = fire_propagate_kernel<512, 2, 2, 4>;
     if (smem > 48 * 1024)
-        FIRE_CUDA_TRY(L, cudaFuncSetAttribute(fire_propagate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const bool prof = L->prof_enabled && L->prof_count < 64;
     if (prof) FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count], st));
-    fire_propagate_kernel<<<grid, threads, smem, st>>>(prm);
+    kernel<<<grid, threads, smem, st>>>(prm);
     FIRE_CUDA_TRY(L, cudaGetLastError());
     if (prof) { FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count + 1], st)); L->prof_count += 1; }
     {

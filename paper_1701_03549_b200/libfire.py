@@ -21,7 +21,7 @@ FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
     "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
-    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_error_string",
+    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
 
@@ -58,6 +58,7 @@ def load() -> C.CDLL:
     lib.fire_launch_count.restype = C.c_int64
     lib.fire_set_launch_geometry.argtypes = [_vp, C.c_int32, C.c_int32]
     lib.fire_set_list_capacity.argtypes = [_vp, C.c_int32, C.c_int32]
+    lib.fire_set_schedule.argtypes = [_vp, C.c_int32]
     lib.fire_set_profiling.argtypes = [_vp, C.c_int32]
     lib.fire_profile_read.argtypes = [_vp, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
     lib.fire_error_string.argtypes = [C.c_int]
@@ -229,6 +230,10 @@ def fire_launch_count(L: Landscape) -> int:
 
 def fire_set_launch_geometry(L: Landscape, threads_per_cta: int = 0, ctas_per_sm: int = 0) -> None:
     _check(load().fire_set_launch_geometry(L.handle, int(threads_per_cta), int(ctas_per_sm)), "fire_set_launch_geometry")
+
+
+def fire_set_schedule(L: Landscape, mode: int = 0) -> None:
+    _check(load().fire_set_schedule(L.handle, int(mode)), "fire_set_schedule")
 
 
 def fire_set_list_capacity(L: Landscape, shared_entries: int = 0, total_entries: int = 0) -> None:

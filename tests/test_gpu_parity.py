@@ -219,9 +219,11 @@ def test_results_do_not_depend_on_launch_geometry_or_list_capacity(request):
     assert (base["burned"] == again["burned"]).all()
     for threads, per_sm, shared, total in [(32, 1, 0, 0), (64, 8, 0, 0), (128, 2, 0, 0), (512, 1, 0, 0), (1024, 1, 0, 0),
                                            (256, 4, 16, 0), (256, 4, 5, 4096), (96, 3, 1, 0),
-                                           (256, 4, 8, 8), (128, 4, 64, 100), (256, 2, 0, 1)]:
+                                           (256, 4, 8, 8), (128, 4, 64, 100), (256, 2, 0, 1), (256, 5, 0, 0), (256, 6, 0, 0),
+                                           (256, 8, 768, 0), (128, 1, 0, 0)]:
         lf.fire_set_launch_geometry(L, threads, per_sm)
         lf.fire_set_list_capacity(L, shared, total)
+        lf.fire_set_schedule(L, (threads // 32 + per_sm) % 2)      # largest-expected-first / batch order
         g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
         ok = (g["burned"] == base["burned"]).all(axis=(1, 2))
         assert ok.all(), f"geometry {(threads, per_sm, shared, total)}: sims {np.flatnonzero(~ok)[:10]} differ"
