@@ -78,9 +78,9 @@ constexpr int kThrTX = 32, kThrTY = 8;
 __device__ __forceinline__ uint32_t fire_threshold_from_x(double x)
 {
     const double e = exp(-x);
-    const double p = __ddiv_rn(1.0, __dadd_rn(1.0, e));                   // Eq. 1
-    const long long t = __double2ll_rn(p * 4294967296.0);                 // exact scaling, ties-to-even (R-11)
-    return (uint32_t)(t > 0xFFFFFFFFll ? 0xFFFFFFFFll : (t < 0 ? 0 : t));
+    const double p = __drcp_rn(__dadd_rn(1.0, e));                        // Eq. 1: 1 / (1 + exp(-x)), correctly rounded reciprocal
+    const unsigned long long t = (unsigned long long)__double2ll_rn(p * 4294967296.0);   // exact scaling, ties-to-even (R-11); 0 <= t <= 2^32
+    return (uint32_t)t - (uint32_t)(t >> 32);                             // min(t, 2^32 - 1)
 }
 
 // x of Eq. 1 for one (target, direction): every operation one IEEE double operation, in the order of C-3
@@ -100,7 +100,7 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
 {
     __shared__ double sb[FIRE_THR_PGROUP][5];
     __shared__ float s_mean[FIRE_THR_PGROUP];
-    __shared__ uint32_t sT[8][kThrTY + 2][kThrTX + 2];                    // [d][source row + 1][source column + 1]
+    __shared__ uint32_t sT2[2][8][kThrTY + 2][kThrTX + 2];                // [buffer][d][source row + 1][source column + 1]
     const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
     const int p0 = blockIdx.y * FIRE_THR_PGROUP;
     const int np = min(FIRE_THR_PGROUP, P - p0);
@@ -131,6 +131,7 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
     __syncthreads();
     for (int q = 0; q < np; ++q) {
         const double b0 = sb[q][0], b1 = sb[q][1], b2 = sb[q][2], b3 = sb[q][3], b4 = sb[q][4];
+        uint32_t (*sT)[kThrTY + 2][kThrTX + 2] = sT2[q & 1];         // double-buffered: one barrier per parameter vector
         float fsum = 0.0f;
 #pragma unroll
         for (int d = 0; d < 8; ++d) {
@@ -169,8 +170,8 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
                 }
             }
         }
-        __syncthreads();
     }
+    __syncthreads();
     if (tid < np) atomicAdd(param_mean + p0 + tid, s_mean[tid]);
 }
 

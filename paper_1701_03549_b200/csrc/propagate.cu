@@ -227,12 +227,17 @@ struct philox_step {
     uint32_t x1, y1, a1l;
 };
 
-// Phase 2 for K units of 32 trials (units u0, u0 + ustride, ...; all of them exist: u * 32 < nQ).
-// Stages, so that each long latency is waited for once per pass: queue reads -> Philox -> atomics -> compaction.
+// Phase 2 for K units of 32 trials (units u0, u0 + ustride, ...; all of them exist: u * 32 < nQ), in two halves so
+// that the caller can overlap the atomics of one pass with the arithmetic of the next:
+//   trials_issue  : queue reads -> Philox -> compare -> atomicAnd on the susceptible plane (results left pending)
+//   trials_resolve: the lane whose atomic saw the bit still set owns the new burning cell -> next frontier
+template <int K> struct pending_trials { uint32_t item[K], bit[K], old[K]; };
+
 template <int K>
-__device__ __forceinline__ void trials_pass(const step_ctx& c, const philox_step& ph, uint32_t u0, uint32_t ustride)
+__device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_step& ph, uint32_t u0, uint32_t ustride,
+                                             pending_trials<K>& pt)
 {
-    uint32_t item[K], T[K];
+    uint32_t T[K];
     const bool q_shared = (u0 + (uint32_t)(K - 1) * ustride + 1u) * 32u <= c.capQ_s;      // warp-uniform
 #pragma unroll
     for (int u = 0; u < K; ++u) {
@@ -240,17 +245,15 @@ __device__ __forceinline__ void trials_pass(const step_ctx& c, const philox_step
         const bool live = j < c.nQ;
         j = live ? j : c.nQ - 1u;
         const uint2 it = (q_shared || j < c.capQ_s) ? lds64(c.qs_addr + 8u * j) : __ldcg(c.Qg + (j - c.capQ_s));
-        item[u] = it.x;
+        pt.item[u] = it.x;
         T[u] = live ? it.y : 0u;                                   // T = 0 never succeeds
     }
-    bool succ[K];
-    uint32_t widx[K], bit[K], old[K];
 #pragma unroll
     for (int u = 0; u < K; ++u) {
-        const uint32_t ty = item[u] >> 16, tx = (item[u] >> 3) & 0x1FFFu, d = item[u] & 7u;
+        const uint32_t ty = pt.item[u] >> 16, tx = (pt.item[u] >> 3) & 0x1FFFu, d = pt.item[u] & 7u;
         const uint32_t cell = ty * c.W + tx;
-        bit[u] = ((ty & 3u) << 3) | (tx & 7u);
-        widx[u] = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
+        pt.bit[u] = ((ty & 3u) << 3) | (tx & 7u);
+        const uint32_t widx = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
         // round 0: (cell, t, sim, d >> 2) -> (r0c0, bl, hi(cell * M0) ^ (d >> 2) ^ k1, lo(cell * M0))
         uint32_t c3 = cell * kM0;
         uint32_t c2 = __umulhi(cell, kM0) ^ (d >> 2) ^ ph.rk1[0];
@@ -269,21 +272,24 @@ __device__ __forceinline__ void trials_pass(const step_ctx& c, const philox_step
         }
         const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
         const uint32_t rnd = (d & 2u) ? hi : lo;
-        succ[u] = fire_trial(rnd, T[u]);
-    }
-#pragma unroll
-    for (int u = 0; u < K; ++u) {
-        old[u] = 0u;
-        if (succ[u]) old[u] = atomicAnd(c.sus32 + widx[u], ~(1u << bit[u]));
+        pt.old[u] = 0u;
+        if (fire_trial(rnd, T[u])) {
+            pt.old[u] = atomicAnd(c.sus32 + widx, ~(1u << pt.bit[u]));
 #ifdef FIRE_PREFETCH_THR
-        if (succ[u]) asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)((((item[u] >> 16) * c.W + ((item[u] >> 3) & 0x1FFFu))) * 2u)));
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)(cell * 2u)));
 #endif
+        }
     }
+}
+
+template <int K>
+__device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_trials<K>& pt)
+{
     uint32_t fresh_mask[K];
     uint32_t n_fresh = 0;
 #pragma unroll
     for (int u = 0; u < K; ++u) {
-        fresh_mask[u] = __ballot_sync(0xFFFFFFFFu, (old[u] >> bit[u]) & 1u);     // old = 0 unless the trial succeeded
+        fresh_mask[u] = __ballot_sync(0xFFFFFFFFu, (pt.old[u] >> pt.bit[u]) & 1u);     // old = 0 unless the trial succeeded
         n_fresh += __popc(fresh_mask[u]);
     }
     if (n_fresh == 0) return;                                      // warp-uniform
@@ -293,7 +299,7 @@ __device__ __forceinline__ void trials_pass(const step_ctx& c, const philox_step
     if (abase + n_fresh <= c.capA_s) {                             // warp-uniform: all new cells go to shared memory
 #pragma unroll
         for (int u = 0; u < K; ++u) {
-            const uint32_t en = (item[u] & 0xFFFF0000u) | ((item[u] >> 3) & 0x1FFFu);
+            const uint32_t en = (pt.item[u] & 0xFFFF0000u) | ((pt.item[u] >> 3) & 0x1FFFu);
             const uint32_t a = c.an_addr + 4u * (abase + __popc(fresh_mask[u] & c.lt));
             if (fresh_mask[u] & (1u << c.lane)) sts32(a, en);
             abase += __popc(fresh_mask[u]);
@@ -303,7 +309,7 @@ __device__ __forceinline__ void trials_pass(const step_ctx& c, const philox_step
         for (int u = 0; u < K; ++u) {
             if (fresh_mask[u] & (1u << c.lane)) {
                 const uint32_t pos = abase + __popc(fresh_mask[u] & c.lt);
-                const uint32_t en = (item[u] & 0xFFFF0000u) | ((item[u] >> 3) & 0x1FFFu);
+                const uint32_t en = (pt.item[u] & 0xFFFF0000u) | ((pt.item[u] >> 3) & 0x1FFFu);
                 if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, en);
                 else if (pos < c.capA) __stcg(c.An_g + (pos - c.capA_s), en);
                 else *c.over = 1u;
@@ -425,10 +431,24 @@ fire_propagate_kernel(const prop_params prm)
                 ph.y1 = __umulhi(r0c0, kM0) ^ ph.rk1[1];
                 const uint32_t nU = (c.nQ + 31u) >> 5;
                 uint32_t u = warp;
-                if (kTrialsInFlight > 1)
-                    for (; u + (uint32_t)(kTrialsInFlight - 1) * nwarps < nU; u += nwarps * kTrialsInFlight)
-                        trials_pass<kTrialsInFlight>(c, ph, u, nwarps);
-                for (; u < nU; u += nwarps) trials_pass<1>(c, ph, u, nwarps);
+                // full passes of kTrialsInFlight units, software-pipelined: the atomics of a pass are resolved after the
+                // arithmetic of the next pass has been issued; then the remaining single units
+                if (kTrialsInFlight > 1) {
+                    pending_trials<kTrialsInFlight> prev;
+                    bool have = false;
+                    for (; u + (uint32_t)(kTrialsInFlight - 1) * nwarps < nU; u += nwarps * kTrialsInFlight) {
+                        pending_trials<kTrialsInFlight> cur;
+                        trials_issue<kTrialsInFlight>(c, ph, u, nwarps, cur);
+                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
+                        prev = cur; have = true;
+                    }
+                    if (have) trials_resolve<kTrialsInFlight>(c, prev);
+                }
+                for (; u < nU; u += nwarps) {
+                    pending_trials<1> cur;
+                    trials_issue<1>(c, ph, u, nwarps, cur);
+                    trials_resolve<1>(c, cur);
+                }
             }
             __syncthreads();
             ++t;
@@ -805,7 +825,10 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         kernel = variant == 1 ? fire_propagate_kernel<256, 5, 1, 2> : (variant == 2 ? fire_propagate_kernel<256, 5, 1, 4> : fire_propagate_kernel<256, 5, 2, 4>);
     else if (threads <= 256)
         kernel = variant == 2 ? fire_propagate_kernel<256, 4, 1, 4> : fire_propagate_kernel<256, 4, 2, 4>;
+    else if (threads <= 512 && per_sm >= 4) kernel = variant == 1 ? fire_propagate_kernel<512, 4, 1, 1> : fire_propagate_kernel<512, 4, 1, 2>;
+    else if (threads <= 512 && per_sm == 3) kernel = fire_propagate_kernel<512, 3, 1, 4>;
     else if (threads <= 512) kernel = fire_propagate_kernel<512, 2, 2, 4>;
+    else if (per_sm >= 2) kernel = fire_propagate_kernel<1024, 2, 1, 2>;
     if (smem > 48 * 1024)
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const bool prof = L->prof_enabled && L->prof_count < 64;
