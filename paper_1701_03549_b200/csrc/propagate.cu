@@ -99,6 +99,10 @@ __device__ __forceinline__ uint2 lds64(uint32_t addr)
 {
     uint2 v; asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory"); return v;
 }
+__device__ __forceinline__ uint32_t atoms_add(uint32_t addr, uint32_t v)
+{
+    uint32_t old; asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory"); return old;
+}
 __device__ __forceinline__ uint32_t lds32(uint32_t addr)
 {
     uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
@@ -123,7 +127,7 @@ struct step_ctx {
     uint32_t qs_addr, ac_addr, an_addr;   // shared-window addresses: trial queue, current frontier, next frontier
     uint32_t capQ_s, capA_s, capA;
     uint2* Qg; const uint32_t* Ac_g; uint32_t* An_g;
-    unsigned int* cntQ; unsigned int* cntA_next; unsigned int* over;
+    uint32_t cntQ, cntA_next, over;       // shared-window addresses of the queue counter, the next frontier's counter, the overflow flag
     uint32_t nA, nQ;
     uint32_t lane, lt;
 };
@@ -187,7 +191,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
     const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
     if (total == 0) return 0u;
     uint32_t qbase = 0;
-    if (c.lane == 31) qbase = atomicAdd(c.cntQ, total);
+    if (c.lane == 31) qbase = atoms_add(c.cntQ, total);
     qbase = __shfl_sync(0xFFFFFFFFu, qbase, 31);
     uint32_t pos = qbase + incl - cnt;
     if (qbase + total <= c.capQ_s) {                                  // warp-uniform: the whole batch fits in shared memory
@@ -294,7 +298,7 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
     }
     if (n_fresh == 0) return;                                      // warp-uniform
     uint32_t abase = 0;
-    if (c.lane == 0) abase = atomicAdd(c.cntA_next, n_fresh);
+    if (c.lane == 0) abase = atoms_add(c.cntA_next, n_fresh);
     abase = __shfl_sync(0xFFFFFFFFu, abase, 0);
     if (abase + n_fresh <= c.capA_s) {                             // warp-uniform: all new cells go to shared memory
 #pragma unroll
@@ -312,7 +316,7 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
                 const uint32_t en = (pt.item[u] & 0xFFFF0000u) | ((pt.item[u] >> 3) & 0x1FFFu);
                 if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, en);
                 else if (pos < c.capA) __stcg(c.An_g + (pos - c.capA_s), en);
-                else *c.over = 1u;
+                else sts32(c.over, 1u);
             }
             abase += __popc(fresh_mask[u]);
         }
@@ -347,7 +351,8 @@ fire_propagate_kernel(const prop_params prm)
     c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th;
     c.qs_addr = qs_addr; c.capQ_s = prm.capQ_s; c.capA_s = prm.capA_s; c.capA = prm.capA;
     c.Qg = reinterpret_cast<uint2*>(prm.spill + (size_t)blockIdx.x * spill_per_cta);
-    c.over = &s_over;
+    c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
+    const uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]), cntQ_addr = (uint32_t)__cvta_generic_to_shared(&s_cntQ[0]);
     c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
 
     for (;;) {
@@ -396,7 +401,7 @@ fire_propagate_kernel(const prop_params prm)
             const uint32_t par = t & 1u;
             c.ac_addr = par ? as_addr1 : as_addr0; c.an_addr = par ? as_addr0 : as_addr1;
             c.Ac_g = par ? Ag1 : Ag0; c.An_g = par ? Ag0 : Ag1;
-            c.cntQ = &s_cntQ[par]; c.cntA_next = &s_cntA[par ^ 1u];
+            c.cntQ = cntQ_addr + 4u * par; c.cntA_next = cntA_addr + 4u * (par ^ 1u);
 
             // ---- phase 1: susceptible neighbours of the burning cells and their thresholds -> trial queue.
             // Units of 32 cells are dealt round-robin to the warps: full passes of kCellsInFlight units, then single units.
