@@ -39,7 +39,8 @@ struct prop_params {
     const uint64_t* seeds;        // [S]
     const int32_t*  sim_ids;      // [S] or null
     const uint32_t* order;        // [S] launch order or null
-    uint64_t* tiles;              // [S][Th][Tw] susceptible planes
+    uint64_t* tiles;              // [S][planes][Th][Tw] susceptible planes (planes = 1, or 2 for the asynchronous-warp kernel)
+    uint32_t* plane_sel;          // [S] which plane holds the final state (asynchronous-warp kernel)
     uint32_t* out_burned;         // [S][H][Ww]
     uint32_t* out_steps;          // [S] or null
     unsigned long long* out_trials;  // [S] or null
@@ -479,6 +480,227 @@ fire_propagate_kernel(const prop_params prm)
     }
 }
 
+
+// The same first half for trials taken from a warp's own ring buffer (asynchronous-warp kernel): n <= 32 entries at `head`.
+__device__ __forceinline__ void trials_issue_ring(const step_ctx& c, const philox_step& ph, uint32_t ring_addr, uint32_t head,
+                                                  uint32_t n, uint32_t ring_mask, pending_trials<1>& pt)
+{
+    const bool live = c.lane < n;
+    const uint2 it = lds64(ring_addr + 8u * ((head + (live ? c.lane : 0u)) & ring_mask));
+    pt.item[0] = it.x;
+    const uint32_t T = live ? it.y : 0u;                           // T = 0 never succeeds
+    const uint32_t ty = it.x >> 16, tx = (it.x >> 3) & 0x1FFFu, d = it.x & 7u;
+    const uint32_t cell = ty * c.W + tx;
+    pt.bit[0] = ((ty & 3u) << 3) | (tx & 7u);
+    const uint32_t widx = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
+    uint32_t c3 = cell * kM0;
+    uint32_t c2 = __umulhi(cell, kM0) ^ (d >> 2) ^ ph.rk1[0];
+    uint32_t c0 = __umulhi(c2, kM1) ^ ph.x1;
+    uint32_t c1 = c2 * kM1;
+    c2 = ph.y1 ^ c3;
+    c3 = ph.a1l;
+#pragma unroll
+    for (int r = 2; r < 10; ++r) {
+        const uint64_t a = (uint64_t)c0 * kM0;
+        const uint64_t b = (uint64_t)c2 * kM1;
+        const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ ph.rk0[r];
+        const uint32_t n2 = (uint32_t)(a >> 32) ^ c3 ^ ph.rk1[r];
+        c1 = (uint32_t)b; c3 = (uint32_t)a; c0 = n0; c2 = n2;
+    }
+    const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
+    const uint32_t rnd = (d & 2u) ? hi : lo;
+    pt.old[0] = 0u;
+    if (fire_trial(rnd, T)) pt.old[0] = atomicAnd(c.sus32 + widx, ~(1u << pt.bit[0]));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Asynchronous-warp kernel: ONE block barrier per CA step.
+// Two susceptible planes per simulation: step t READS plane t & 1 (exactly the state at the start of the step) and
+// UPDATES plane (t + 1) & 1, which lags by the cells that are burning now; every burning cell first clears its own bit
+// there ("catch-up", a fire-and-forget reduction), so that after the step the written plane is exactly the state at
+// the start of step t + 1.  A successful trial's atomicAnd on the written plane still says who ignited the cell first.
+// Because nothing read in a step is written in that step, there is no barrier between building trials and running
+// them: every warp takes units of 32 burning cells, appends their trials to its OWN ring buffer in shared memory and
+// runs them 32 at a time as soon as it has them; the loads of the next cell unit are in flight meanwhile.
+// ------------------------------------------------------------------------------------------------
+constexpr uint32_t kRingEntries = 512;             // per warp, 8 B each: one cell unit adds at most 256 trials to at most 31 left over
+
+template <int kMaxThreads, int kMinCtas>
+__global__ void __launch_bounds__(kMaxThreads, kMinCtas)
+fire_propagate_async_kernel(const prop_params prm)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    const int tid = threadIdx.x;
+    const uint32_t warp = (uint32_t)tid >> 5, nwarps = blockDim.x >> 5;
+    // shared layout: per-warp trial rings, frontier list 0, frontier list 1
+    uint32_t ring_addr = (uint32_t)__cvta_generic_to_shared(smem) + warp * (kRingEntries * 8u);
+    asm volatile("" : "+r"(ring_addr));
+    const uint32_t as_addr0 = (uint32_t)__cvta_generic_to_shared(smem) + nwarps * (kRingEntries * 8u), as_addr1 = as_addr0 + 4u * prm.capA_s;
+    const size_t spill_per_cta = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);
+    uint32_t* const Ag0 = prm.spill + (size_t)blockIdx.x * spill_per_cta + (size_t)2 * (prm.capQ - prm.capQ_s);
+    uint32_t* const Ag1 = Ag0 + (prm.capA - prm.capA_s);
+
+    __shared__ unsigned int s_sim, s_cntA[3], s_over;
+    __shared__ unsigned long long s_trials;
+
+    step_ctx c;
+    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th;
+    c.capA_s = prm.capA_s; c.capA = prm.capA; c.capQ_s = 0u; c.qs_addr = 0u; c.Qg = nullptr; c.cntQ = 0u; c.nQ = 0u;
+    c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
+    const uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]);
+    c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
+    const size_t nt = (size_t)c.Tw * c.Th;
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) {
+            const unsigned int k = atomicAdd(prm.work_counter, 1u);
+            s_sim = (k < (unsigned int)prm.S) ? (prm.order ? prm.order[k] : k) : 0xFFFFFFFFu;
+        }
+        __syncthreads();
+        const uint32_t s = s_sim;
+        if (s == 0xFFFFFFFFu) break;
+#ifdef FIRE_TRACE
+        unsigned long long trace_t0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t0));
+#endif
+        const int p = prm.sim_param[s];
+        const int ix = prm.ignitions[2 * s], iy = prm.ignitions[2 * s + 1];
+        const uint64_t seed = prm.seeds[s];
+        const uint32_t sim = prm.sim_ids ? (uint32_t)prm.sim_ids[s] : s;
+        uint64_t* const plane0 = prm.tiles + (size_t)s * 2 * nt;
+        bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
+        if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
+        c.thr4 = reinterpret_cast<const uint4*>(prm.thr + (valid ? (size_t)p * c.W * prm.H * 8 : 0));
+        const uint32_t key_lo = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)seed), key_hi = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)(seed >> 32));
+        const uint32_t bh = __umulhi(sim, kM1), bl = sim * kM1;
+
+        if (tid == 0) {
+            s_cntA[0] = valid ? 1u : 0u; s_cntA[1] = 0u; s_cntA[2] = 0u; s_over = 0u; s_trials = 0ull;
+            if (valid) {
+                const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
+                if (prm.capA_s > 0) sts32(as_addr0, e0); else Ag0[0] = e0;
+                // the ignition is burnt at t = 0: cleared in plane 0 (read by step 0); plane 1 is caught up by step 0 itself
+                atomicAnd(reinterpret_cast<uint32_t*>(plane0) + (((size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
+            }
+        }
+        __syncthreads();
+
+        uint32_t t = 0, my_trials = 0;
+        c.nA = valid ? 1u : 0u;
+        bool over = false;
+        while (c.nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
+            const uint32_t par = t & 1u;
+            c.ac_addr = par ? as_addr1 : as_addr0; c.an_addr = par ? as_addr0 : as_addr1;
+            c.Ac_g = par ? Ag1 : Ag0; c.An_g = par ? Ag0 : Ag1;
+            c.cntA_next = cntA_addr + 4u * ((t + 1u) % 3u);
+            if (tid == 0) s_cntA[(t + 2u) % 3u] = 0u;             // read last at the start of step t - 1, appended to in step t + 1
+            c.sus = plane0 + (size_t)par * nt;                                              // read plane
+            c.sus32 = reinterpret_cast<uint32_t*>(plane0 + (size_t)(par ^ 1u) * nt);        // written plane
+
+            philox_step ph;
+#pragma unroll
+            for (int r = 0; r < 10; ++r) { ph.rk0[r] = key_lo + (uint32_t)r * kW0; ph.rk1[r] = key_hi + (uint32_t)r * kW1; }
+            const uint32_t r0c0 = bh ^ t ^ ph.rk0[0];
+            ph.a1l = r0c0 * kM0; ph.x1 = bl ^ ph.rk0[1]; ph.y1 = __umulhi(r0c0, kM0) ^ ph.rk1[1];
+
+            uint32_t head = 0, fill = 0;                           // this warp's ring: entries [head, head + fill) mod kRingEntries
+            pending_trials<1> prev; bool have = false;
+            const uint32_t nU = (c.nA + 31u) >> 5;
+            for (uint32_t u = warp; u < nU; u += nwarps) {
+                // ---- one unit of 32 burning cells: window, thresholds, catch-up, trials appended to the ring
+                uint32_t i = u * 32u + c.lane;
+                const bool live = i < c.nA;
+                i = live ? i : c.nA - 1u;
+                const uint32_t e = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.Ac_g + (i - c.capA_s));
+                const uint32_t x = e & 0xFFFFu, y = e >> 16;
+                const uint32_t tx0 = x >> 3, ty0 = y >> 3, bx = x & 7u, by = y & 7u;
+                const uint32_t tidx = ty0 * c.Tw + tx0;
+                const int hoff = (bx == 0u && tx0 > 0u) ? -1 : ((bx == 7u && tx0 + 1u < c.Tw) ? 1 : 0);
+                const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
+                const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
+                const uint64_t tc = ldcg_u64(c.sus + tidx);
+                const uint4 Ta = ldg_thr(sp), Tb = ldg_thr(sp + 1);
+                uint64_t th = 0ull, tv = 0ull, td = 0ull;
+                if (hoff) th = ldcg_u64(c.sus + (tidx + hoff));
+                if (voff) tv = ldcg_u64(c.sus + (tidx + voff));
+                if (hoff && voff) td = ldcg_u64(c.sus + (tidx + hoff + voff));
+                if (live) atomicAnd(c.sus32 + ((tidx << 1) | ((y >> 2) & 1u)), ~(1u << (((y & 3u) << 3) | bx)));      // catch-up (no return: RED)
+
+                // while those loads are in flight: run the trials already in the ring
+                while (fill >= 32u) {
+                    pending_trials<1> cur;
+                    trials_issue_ring(c, ph, ring_addr, head, 32u, kRingEntries - 1u, cur);
+                    if (have) trials_resolve<1>(c, prev);
+                    prev = cur; have = true;
+                    head = (head + 32u) & (kRingEntries - 1u); fill -= 32u;
+                }
+
+                const uint32_t selr = ((by + 7u) & 7u) | (by << 4) | (((by + 1u) & 7u) << 8);
+                uint32_t w3c = __byte_perm((uint32_t)tc, (uint32_t)(tc >> 32), selr) & 0xFFFFFFu;
+                uint32_t w3h = __byte_perm((uint32_t)th, (uint32_t)(th >> 32), selr) & 0xFFFFFFu;
+                const uint32_t vc = (by == 0u) ? (uint32_t)(tv >> 56) : (((uint32_t)tv & 0xFFu) << 16);
+                const uint32_t vh = (by == 0u) ? (uint32_t)(td >> 56) : (((uint32_t)td & 0xFFu) << 16);
+                const uint32_t keep = (by == 0u) ? 0xFFFF00u : ((by == 7u) ? 0x00FFFFu : 0xFFFFFFu);
+                w3c = (w3c & keep) | vc;
+                w3h = (w3h & keep) | vh;
+                const uint32_t tcen = (w3c << 1) >> bx;
+                const uint32_t mC = (bx == 0u) ? 0x060606u : ((bx == 7u) ? 0x030303u : 0x070707u);
+                const uint32_t hb = (bx == 0u) ? ((w3h >> 7) & 0x010101u) : ((w3h << 2) & 0x040404u);
+                const uint32_t w = live ? ((tcen & mC) | hb) : 0u;
+                const uint32_t cnt = __popc(w);
+                uint32_t incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                    if (c.lane >= (uint32_t)o) incl += v;
+                }
+                const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                my_trials += cnt;
+                const uint32_t pos = head + fill + incl - cnt;
+                const uint32_t base = ((e & 0xFFFFu) << 3) | (e & 0xFFFF0000u);
+#define FIRE_EMIT(bit, d, Tv) \
+                if (w & (1u << (bit))) sts64(ring_addr + 8u * ((pos + __popc(w & ((1u << (bit)) - 1u))) & (kRingEntries - 1u)), base + item_delta(d), (Tv));
+                FIRE_EMIT(0, 7, Tb.w)  FIRE_EMIT(1, 0, Ta.x)  FIRE_EMIT(2, 1, Ta.y)
+                FIRE_EMIT(8, 6, Tb.z)  FIRE_EMIT(10, 2, Ta.z)
+                FIRE_EMIT(16, 5, Tb.y) FIRE_EMIT(17, 4, Tb.x) FIRE_EMIT(18, 3, Ta.w)
+#undef FIRE_EMIT
+                fill += total;
+                __syncwarp();
+            }
+            // ---- the rest of the ring, last unit possibly partial
+            while (fill > 0u) {
+                const uint32_t n = fill < 32u ? fill : 32u;
+                pending_trials<1> cur;
+                trials_issue_ring(c, ph, ring_addr, head, n, kRingEntries - 1u, cur);
+                if (have) trials_resolve<1>(c, prev);
+                prev = cur; have = true;
+                head = (head + n) & (kRingEntries - 1u); fill -= n;
+            }
+            if (have) trials_resolve<1>(c, prev);
+            __syncthreads();
+            ++t;
+            if (s_over) { over = true; break; }
+            c.nA = s_cntA[t % 3u];
+        }
+
+        if (my_trials) atomicAdd(&s_trials, (unsigned long long)my_trials);
+        __syncthreads();
+        if (tid == 0) {
+            if (over) {
+                prm.rescue_list[atomicAdd(prm.work_counter + 1, 1u)] = s;
+            } else {
+                prm.plane_sel[s] = t & 1u;                         // the plane that holds the final state
+                if (prm.out_steps) prm.out_steps[s] = t;
+                if (prm.out_trials) prm.out_trials[s] = s_trials;
+#ifdef FIRE_TRACE
+                unsigned long long trace_t1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t1));
+                if (prm.out_trials) prm.out_trials[s] = (((trace_t0 / 1000ull) & 0xFFFFFFFFull) << 32) | (((trace_t1 - trace_t0) / 1000ull) & 0xFFFFFFFFull);
+#endif
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // Plane set-up and tear-down around the fast kernel (pure streams).
 //   fire_burnable_tiles_kernel : once per landscape, burnable bitmap -> tile layout
@@ -515,13 +737,14 @@ fire_init_tiles_kernel(const uint64_t* __restrict__ burnable_tiles, uint64_t* __
 
 // one thread per (tile row, bitmap word column): 4 tiles in (32 B), 8 words out (one per lattice row)
 __global__ void __launch_bounds__(256)
-fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __restrict__ tiles, uint32_t* __restrict__ out_burned,
-                   int H, int Ww, int Tw, int Th)
+fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __restrict__ tiles, const uint32_t* __restrict__ plane_sel,
+                   int planes, uint32_t* __restrict__ out_burned, int H, int Ww, int Tw, int Th)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Th * Ww) return;
     const int ty = i / Ww, wx = i % Ww;
-    const uint64_t* const row = tiles + (size_t)blockIdx.y * Tw * Th + (size_t)ty * Tw;
+    const size_t plane = (size_t)blockIdx.y * planes + (planes > 1 ? (plane_sel[blockIdx.y] & 1u) : 0u);
+    const uint64_t* const row = tiles + plane * Tw * Th + (size_t)ty * Tw;
     uint64_t tl[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) tl[k] = (4 * wx + k < Tw) ? __ldcs(reinterpret_cast<const unsigned long long*>(row + 4 * wx + k)) : 0ull;
@@ -755,7 +978,15 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     prm.capQ = 8u * capA;
     prm.capQ_s = 2u * capA_s;                                  // default: 1536-cell lists + 3072-trial queue = 36 KiB per CTA
     if (prm.capQ_s > prm.capQ) prm.capQ_s = prm.capQ;
-    const size_t smem = ((size_t)2 * prm.capA_s + (size_t)2 * prm.capQ_s) * sizeof(uint32_t);
+    // kernel family: 0 = two-phase kernel (one state plane, two barriers per step); 1 = asynchronous-warp kernel
+    // (two state planes, one barrier per step, per-warp trial rings)
+    // Default: the two-phase kernel for batches that fill the GPU with 256-thread CTAs; the asynchronous-warp kernel for
+    // small batches of large fires (wide CTAs), whose trial queues would not fit in shared memory.  fire_set_schedule
+    // bits 4.. force one: 8 = asynchronous-warp, 9 = two-phase.
+    const bool async = L->kernel_variant == 8 || (L->kernel_variant != 9 && L->kernel_variant < 8 && threads >= 512 && L->threads_per_cta == 0);
+    const int planes = async ? 2 : 1;
+    const size_t smem = async ? ((size_t)(threads / 32) * kRingEntries * 8 + (size_t)2 * prm.capA_s * sizeof(uint32_t))
+                              : ((size_t)2 * prm.capA_s + (size_t)2 * prm.capQ_s) * sizeof(uint32_t);
     if (smem > 200 * 1024) return FIRE_EINVAL;
 
     // ---- scratch owned by the handle (grow-only; growing waits for the stream first)
@@ -764,12 +995,12 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     const size_t nw = (size_t)L->H * L->Ww;
     const size_t nt = (size_t)L->Tw * L->Th;
     const size_t rescue_bytes = nw * 4 * 2 * kRescueCtas;
-    const size_t tiles_bytes = nt * 8 * (size_t)S;
-    if (L->status_capacity < (size_t)S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes ||
+    const size_t tiles_bytes = nt * 8 * (size_t)S * 2;        // room for two planes per simulation
+    if (L->status_capacity < (size_t)2 * S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes ||
         L->tiles_capacity < tiles_bytes || L->order_capacity < (size_t)S * 4 || L->burnable_tiles == nullptr) {
         FIRE_CUDA_TRY(L, cudaStreamSynchronize(st));
         size_t cap_bytes = L->status_capacity * 4;
-        int rc = fire_reserve(L, (void**)&L->status, &cap_bytes, (size_t)S * 4);
+        int rc = fire_reserve(L, (void**)&L->status, &cap_bytes, (size_t)2 * S * 4);     // rescue list [S] + plane selector [S]
         if (rc != FIRE_OK) return rc;
         L->status_capacity = cap_bytes / 4;
         rc = fire_reserve(L, (void**)&L->spill, &L->spill_capacity, spill_bytes);
@@ -795,7 +1026,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
 
     prm.burnable = L->burnable; prm.thr = L->thr;
     prm.ignitions = ignitions; prm.sim_param = sim_param; prm.seeds = seeds; prm.sim_ids = sim_ids;
-    prm.tiles = L->tiles;
+    prm.tiles = L->tiles; prm.plane_sel = L->status + S;
     prm.out_burned = out_burned; prm.out_steps = out_steps; prm.out_trials = (unsigned long long*)out_trials;
     prm.work_counter = L->work_counter; prm.rescue_list = L->status; prm.spill = L->spill;
     prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.Tw = L->Tw; prm.Th = L->Th;
@@ -816,10 +1047,11 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         unsigned chunks = (unsigned)((units + 256 * 4 - 1) / (256 * 4));
         if (chunks < 1) chunks = 1;
         if (chunks > 64) chunks = 64;
-        fire_init_tiles_kernel<<<dim3(chunks, (unsigned)S), 256, 0, st>>>(L->burnable_tiles, L->tiles, nt);
+        fire_init_tiles_kernel<<<dim3(chunks, (unsigned)(S * planes)), 256, 0, st>>>(L->burnable_tiles, L->tiles, nt);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
     FIRE_CUDA_TRY(L, cudaMemsetAsync(L->work_counter, 0, 2 * sizeof(unsigned int), st));
+    if (async) FIRE_CUDA_TRY(L, cudaMemsetAsync(L->status + S, 0, (size_t)S * 4, st));
     void (*kernel)(const prop_params) = fire_propagate_kernel<1024, 1, 2, 4>;
     const int variant = L->kernel_variant;
     if (threads <= 256 && per_sm >= 8)
@@ -834,7 +1066,14 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     else if (threads <= 512 && per_sm == 3) kernel = fire_propagate_kernel<512, 3, 1, 4>;
     else if (threads <= 512) kernel = fire_propagate_kernel<512, 2, 2, 4>;
     else if (per_sm >= 2) kernel = fire_propagate_kernel<1024, 2, 1, 2>;
-    if (smem > 48 * 1024)
+    if (async) {
+        if (threads <= 256 && per_sm >= 6) kernel = fire_propagate_async_kernel<256, 6>;
+        else if (threads <= 256 && per_sm == 5) kernel = fire_propagate_async_kernel<256, 5>;
+        else if (threads <= 256) kernel = fire_propagate_async_kernel<256, 4>;
+        else if (threads <= 512) kernel = fire_propagate_async_kernel<512, 2>;
+        else kernel = fire_propagate_async_kernel<1024, 1>;
+    }
+    if (smem + 1024 > 48 * 1024)                     // dynamic + static shared memory beyond the default limit
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const bool prof = L->prof_enabled && L->prof_count < 64;
     if (prof) FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count], st));
@@ -843,7 +1082,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     if (prof) { FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count + 1], st)); L->prof_count += 1; }
     {
         const size_t n = (size_t)L->Th * L->Ww;
-        fire_finish_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)S), 256, 0, st>>>(L->burnable, L->tiles, out_burned,
+        fire_finish_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)S), 256, 0, st>>>(L->burnable, L->tiles, L->status + S, planes, out_burned,
                                                                                           L->H, L->Ww, L->Tw, L->Th);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }

@@ -217,17 +217,20 @@ def test_results_do_not_depend_on_launch_geometry_or_list_capacity(request):
     base = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
     again = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
     assert (base["burned"] == again["burned"]).all()
-    for threads, per_sm, shared, total in [(32, 1, 0, 0), (64, 8, 0, 0), (128, 2, 0, 0), (512, 1, 0, 0), (1024, 1, 0, 0),
-                                           (256, 4, 16, 0), (256, 4, 5, 4096), (96, 3, 1, 0),
-                                           (256, 4, 8, 8), (128, 4, 64, 100), (256, 2, 0, 1), (256, 5, 0, 0), (256, 6, 0, 0),
-                                           (256, 8, 768, 0), (128, 1, 0, 0)]:
+    # mode: bit 0 = batch order instead of largest-expected-first; 128 / 144 force the asynchronous-warp / two-phase kernel
+    for threads, per_sm, shared, total, mode in [(32, 1, 0, 0, 0), (64, 8, 0, 0, 1), (128, 2, 0, 0, 0), (512, 1, 0, 0, 144), (1024, 1, 0, 0, 145),
+                                                 (256, 4, 16, 0, 0), (256, 4, 5, 4096, 1), (96, 3, 1, 0, 0), (256, 4, 8, 8, 0),
+                                                 (128, 4, 64, 100, 1), (256, 2, 0, 1, 0), (256, 5, 0, 0, 0), (256, 6, 0, 0, 1),
+                                                 (256, 8, 768, 0, 0), (128, 1, 0, 0, 1),
+                                                 (256, 4, 0, 0, 128), (32, 2, 0, 0, 129), (1024, 1, 0, 0, 128), (512, 2, 16, 0, 128),
+                                                 (256, 5, 5, 4096, 129), (256, 6, 8, 8, 128), (128, 4, 1, 1, 128), (0, 0, 0, 0, 128)]:
         lf.fire_set_launch_geometry(L, threads, per_sm)
         lf.fire_set_list_capacity(L, shared, total)
-        lf.fire_set_schedule(L, (threads // 32 + per_sm) % 2)      # largest-expected-first / batch order
+        lf.fire_set_schedule(L, mode)
         g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
         ok = (g["burned"] == base["burned"]).all(axis=(1, 2))
-        assert ok.all(), f"geometry {(threads, per_sm, shared, total)}: sims {np.flatnonzero(~ok)[:10]} differ"
-        assert (g["steps"] == base["steps"]).all() and (g["trials"] == base["trials"]).all(), (threads, per_sm, shared, total)
+        assert ok.all(), f"geometry {(threads, per_sm, shared, total, mode)}: sims {np.flatnonzero(~ok)[:10]} differ"
+        assert (g["steps"] == base["steps"]).all() and (g["trials"] == base["trials"]).all(), (threads, per_sm, shared, total, mode)
     L.close()
 
 
