@@ -41,7 +41,7 @@ struct fire_landscape {
     size_t    order_capacity;     // bytes
     float*    param_mean;         // [P] mean contagion probability per parameter vector (written by fire_params_upload)
     size_t    param_mean_capacity;
-    unsigned int* work_counter;   // [2] next sim index for the fast kernel / the rescue kernel
+    unsigned int* work_counter;   // [4] simulations taken by the fast kernel, simulations handed to the rescue kernel, 2 spare
     uint32_t* status;             // [S] 0 = finished by the fast kernel, 1 = needs the rescue kernel
     size_t    status_capacity;    // entries
     uint32_t* spill;              // per resident CTA: frontier + success lists beyond shared memory

@@ -246,7 +246,7 @@ extern "C" int fire_landscape_create(fire_landscape** out, const uint8_t* veg, c
     bool ok = cudaMalloc(&L->flags, n) == cudaSuccess && cudaMalloc(&L->uphill, n) == cudaSuccess &&
               cudaMalloc(&L->psi, n * 8) == cudaSuccess && cudaMalloc(&L->tan_slope, n * 8) == cudaSuccess &&
               cudaMalloc(&L->omega, n * 64) == cudaSuccess && cudaMalloc(&L->burnable, nw * 4) == cudaSuccess &&
-              cudaMalloc(&L->work_counter, 2 * sizeof(unsigned int)) == cudaSuccess &&
+              cudaMalloc(&L->work_counter, 4 * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&L->ref_area, 4 * sizeof(uint32_t)) == cudaSuccess;
     if (!ok) { (void)cudaGetLastError(); fire_landscape_destroy(L); return FIRE_ENOMEM; }
     cudaStream_t st = (cudaStream_t)stream;

@@ -44,10 +44,10 @@ struct prop_params {
     uint32_t* out_burned;         // [S][H][Ww]
     uint32_t* out_steps;          // [S] or null
     unsigned long long* out_trials;  // [S] or null
-    unsigned int* work_counter;   // [0] next sim of the fast kernel, [1] number of sims handed to the rescue kernel
+    unsigned int* work_counter;   // [0] sims taken by the fast kernel, [1] sims handed to the rescue kernel, [2], [3] spare
     uint32_t* rescue_list;        // [S]
     uint32_t* spill;              // [grid][2 * (capQ - capQ_s) + 2 * (capA - capA_s)]
-    int S, P, W, H, Ww, Tw, Th;
+    int S, P, W, H, Ww, Tw, Th, num_sms;
     uint32_t max_steps;
     uint32_t capA_s, capQ_s;      // shared-memory entries: each frontier list, the trial queue
     uint32_t capA, capQ;          // total entries (shared + spill); capQ >= 8 * capA
@@ -115,6 +115,18 @@ __device__ __noinline__ void spill_put_q(uint32_t qs_addr, uint2* Qg, uint32_t c
     if (q < capQ_s) sts64(qs_addr + 8u * q, item, T); else __stcg(Qg + (q - capQ_s), make_uint2(item, T));
 }
 
+
+// Next simulation for this CTA, or 0xFFFFFFFF: batch order, or the order written by fire_order_kernel (largest expected
+// fires first).  (Tried and dropped: CTAs of odd waves taking from the tail of the order, so that an SM hosts large and
+// small fires side by side -- the large fires do get faster, 23.3 -> 21.5 ms, but the medium ones then start late and the
+// launch gets longer, 25.6 -> 28.8 ms.)
+__device__ __forceinline__ uint32_t next_simulation(const prop_params& prm)
+{
+    const unsigned int k = atomicAdd(prm.work_counter, 1u);
+    if (k >= (unsigned int)prm.S) return 0xFFFFFFFFu;
+    return prm.order ? prm.order[k] : k;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Per-step context of one simulation (everything the two pass functions need; all warp-invariant).
 // ------------------------------------------------------------------------------------------------
@@ -135,7 +147,7 @@ struct step_ctx {
 
 // Phase 1 for K units of 32 burning cells (units u0, u0 + ustride, ...; all of them exist: u * 32 < nA).
 // Lanes past the end of the list re-read the last entry and contribute nothing.
-template <int K>
+template <int K, bool kPartial>   // kPartial: units past the end of the frontier are skipped (warp-uniform guards)
 __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, uint32_t ustride)
 {
     uint32_t e[K], win[K];
@@ -146,6 +158,11 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
     for (int k = 0; k < K; ++k) {
         uint32_t i = (u0 + (uint32_t)k * ustride) * 32u + c.lane;
         live[k] = i < c.nA;
+        if (kPartial && k > 0 && (u0 + (uint32_t)k * ustride) * 32u >= c.nA) {      // no such unit
+            e[k] = 0u; tc[k] = 0ull; th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
+            Ta[k] = make_uint4(0u, 0u, 0u, 0u); Tb[k] = make_uint4(0u, 0u, 0u, 0u);
+            continue;
+        }
         i = live[k] ? i : c.nA - 1u;
         e[k] = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.Ac_g + (i - c.capA_s));
         const uint32_t x = e[k] & 0xFFFFu, y = e[k] >> 16;
@@ -165,6 +182,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
     uint32_t cnt = 0;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
+        if (kPartial && k > 0 && (u0 + (uint32_t)k * ustride) * 32u >= c.nA) { win[k] = 0u; continue; }
         const uint32_t bx = e[k] & 7u, by = (e[k] >> 16) & 7u;
         // rows y-1, y, y+1 of the cell's tile column (w3c) and of the horizontally adjacent one (w3h), one per byte
         const uint32_t selr = ((by + 7u) & 7u) | (by << 4) | (((by + 1u) & 7u) << 8);
@@ -200,6 +218,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         if (w & (1u << (bit))) sts64(qa + 8u * __popc(w & ((1u << (bit)) - 1u)), base + item_delta(d), (Tv));
 #pragma unroll
         for (int k = 0; k < K; ++k) {
+            if (kPartial && k > 0 && (u0 + (uint32_t)k * ustride) * 32u >= c.nA) continue;
             const uint32_t w = win[k];
             const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
             const uint32_t qa = c.qs_addr + 8u * pos;
@@ -211,7 +230,11 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
 #undef FIRE_EMIT
     } else {
 #define FIRE_EMIT(bit, d, Tv) \
-        if (w & (1u << (bit))) spill_put_q(c.qs_addr, c.Qg, c.capQ_s, pos + __popc(w & ((1u << (bit)) - 1u)), base + item_delta(d), (Tv));
+        if (w & (1u << (bit))) { \
+            const uint32_t q = pos + __popc(w & ((1u << (bit)) - 1u)); \
+            if (q < c.capQ_s) sts64(c.qs_addr + 8u * q, base + item_delta(d), (Tv)); \
+            else __stcg(c.Qg + (q - c.capQ_s), make_uint2(base + item_delta(d), (Tv))); \
+        }
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             const uint32_t w = win[k];
@@ -238,7 +261,7 @@ struct philox_step {
 //   trials_resolve: the lane whose atomic saw the bit still set owns the new burning cell -> next frontier
 template <int K> struct pending_trials { uint32_t item[K], bit[K], old[K]; };
 
-template <int K>
+template <int K, bool kPartial>   // kPartial: units past the end of the queue are skipped (warp-uniform guards)
 __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_step& ph, uint32_t u0, uint32_t ustride,
                                              pending_trials<K>& pt)
 {
@@ -246,7 +269,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
     const bool q_shared = (u0 + (uint32_t)(K - 1) * ustride + 1u) * 32u <= c.capQ_s;      // warp-uniform
 #pragma unroll
     for (int u = 0; u < K; ++u) {
-        uint32_t j = (u0 + (uint32_t)u * ustride) * 32u + c.lane;
+        uint32_t j = (u0 + (uint32_t)u * ustride) * 32u + c.lane;     // (clamped below: a unit past the end re-reads the last entry)
         const bool live = j < c.nQ;
         j = live ? j : c.nQ - 1u;
         const uint2 it = (q_shared || j < c.capQ_s) ? lds64(c.qs_addr + 8u * j) : __ldcg(c.Qg + (j - c.capQ_s));
@@ -255,6 +278,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
     }
 #pragma unroll
     for (int u = 0; u < K; ++u) {
+        if (kPartial && u > 0 && (u0 + (uint32_t)u * ustride) * 32u >= c.nQ) { pt.bit[u] = 0u; pt.old[u] = 0u; continue; }
         const uint32_t ty = pt.item[u] >> 16, tx = (pt.item[u] >> 3) & 0x1FFFu, d = pt.item[u] & 7u;
         const uint32_t cell = ty * c.W + tx;
         pt.bit[u] = ((ty & 3u) << 3) | (tx & 7u);
@@ -358,10 +382,7 @@ fire_propagate_kernel(const prop_params prm)
 
     for (;;) {
         __syncthreads();                       // the previous simulation's last reads of s_* are done
-        if (tid == 0) {
-            const unsigned int k = atomicAdd(prm.work_counter, 1u);
-            s_sim = (k < (unsigned int)prm.S) ? (prm.order ? prm.order[k] : k) : 0xFFFFFFFFu;
-        }
+        if (tid == 0) s_sim = next_simulation(prm);
         __syncthreads();
         const uint32_t s = s_sim;
         if (s == 0xFFFFFFFFu) break;
@@ -409,10 +430,9 @@ fire_propagate_kernel(const prop_params prm)
             {
                 const uint32_t nU = (c.nA + 31u) >> 5;
                 uint32_t u = warp;
-                if (kCellsInFlight > 1)
-                    for (; u + (uint32_t)(kCellsInFlight - 1) * nwarps < nU; u += nwarps * kCellsInFlight)
-                        my_trials += cells_pass<kCellsInFlight>(c, u, nwarps);
-                for (; u < nU; u += nwarps) my_trials += cells_pass<1>(c, u, nwarps);
+                for (; u + (uint32_t)(kCellsInFlight - 1) * nwarps < nU; u += nwarps * kCellsInFlight)
+                    my_trials += cells_pass<kCellsInFlight, false>(c, u, nwarps);
+                if (u < nU) my_trials += cells_pass<kCellsInFlight, true>(c, u, nwarps);
             }
             __syncthreads();
             c.nQ = s_cntQ[par];
@@ -437,23 +457,24 @@ fire_propagate_kernel(const prop_params prm)
                 ph.y1 = __umulhi(r0c0, kM0) ^ ph.rk1[1];
                 const uint32_t nU = (c.nQ + 31u) >> 5;
                 uint32_t u = warp;
-                // full passes of kTrialsInFlight units, software-pipelined: the atomics of a pass are resolved after the
-                // arithmetic of the next pass has been issued; then the remaining single units
-                if (kTrialsInFlight > 1) {
+                // passes of kTrialsInFlight units, software-pipelined: the atomics of a pass are resolved after the
+                // arithmetic of the next pass has been issued; the last pass of a warp may be partial
+                {
                     pending_trials<kTrialsInFlight> prev;
                     bool have = false;
                     for (; u + (uint32_t)(kTrialsInFlight - 1) * nwarps < nU; u += nwarps * kTrialsInFlight) {
                         pending_trials<kTrialsInFlight> cur;
-                        trials_issue<kTrialsInFlight>(c, ph, u, nwarps, cur);
+                        trials_issue<kTrialsInFlight, false>(c, ph, u, nwarps, cur);
+                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
+                        prev = cur; have = true;
+                    }
+                    if (u < nU) {
+                        pending_trials<kTrialsInFlight> cur;
+                        trials_issue<kTrialsInFlight, true>(c, ph, u, nwarps, cur);
                         if (have) trials_resolve<kTrialsInFlight>(c, prev);
                         prev = cur; have = true;
                     }
                     if (have) trials_resolve<kTrialsInFlight>(c, prev);
-                }
-                for (; u < nU; u += nwarps) {
-                    pending_trials<1> cur;
-                    trials_issue<1>(c, ph, u, nwarps, cur);
-                    trials_resolve<1>(c, cur);
                 }
             }
             __syncthreads();
@@ -481,36 +502,45 @@ fire_propagate_kernel(const prop_params prm)
 }
 
 
-// The same first half for trials taken from a warp's own ring buffer (asynchronous-warp kernel): n <= 32 entries at `head`.
+// The same first half for trials taken from a warp's own ring buffer (asynchronous-warp kernel): n <= 64 entries at `head`,
+// as two interleaved units of 32 (the second one is skipped when n <= 32).
 __device__ __forceinline__ void trials_issue_ring(const step_ctx& c, const philox_step& ph, uint32_t ring_addr, uint32_t head,
-                                                  uint32_t n, uint32_t ring_mask, pending_trials<1>& pt)
+                                                  uint32_t n, uint32_t ring_mask, pending_trials<2>& pt)
 {
-    const bool live = c.lane < n;
-    const uint2 it = lds64(ring_addr + 8u * ((head + (live ? c.lane : 0u)) & ring_mask));
-    pt.item[0] = it.x;
-    const uint32_t T = live ? it.y : 0u;                           // T = 0 never succeeds
-    const uint32_t ty = it.x >> 16, tx = (it.x >> 3) & 0x1FFFu, d = it.x & 7u;
-    const uint32_t cell = ty * c.W + tx;
-    pt.bit[0] = ((ty & 3u) << 3) | (tx & 7u);
-    const uint32_t widx = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
-    uint32_t c3 = cell * kM0;
-    uint32_t c2 = __umulhi(cell, kM0) ^ (d >> 2) ^ ph.rk1[0];
-    uint32_t c0 = __umulhi(c2, kM1) ^ ph.x1;
-    uint32_t c1 = c2 * kM1;
-    c2 = ph.y1 ^ c3;
-    c3 = ph.a1l;
+    uint32_t T[2];
 #pragma unroll
-    for (int r = 2; r < 10; ++r) {
-        const uint64_t a = (uint64_t)c0 * kM0;
-        const uint64_t b = (uint64_t)c2 * kM1;
-        const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ ph.rk0[r];
-        const uint32_t n2 = (uint32_t)(a >> 32) ^ c3 ^ ph.rk1[r];
-        c1 = (uint32_t)b; c3 = (uint32_t)a; c0 = n0; c2 = n2;
+    for (int u = 0; u < 2; ++u) {
+        const bool live = c.lane + 32u * u < n;
+        const uint2 it = lds64(ring_addr + 8u * ((head + (live ? c.lane + 32u * u : 0u)) & ring_mask));
+        pt.item[u] = it.x;
+        T[u] = live ? it.y : 0u;                                   // T = 0 never succeeds
+        pt.old[u] = 0u; pt.bit[u] = 0u;
     }
-    const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
-    const uint32_t rnd = (d & 2u) ? hi : lo;
-    pt.old[0] = 0u;
-    if (fire_trial(rnd, T)) pt.old[0] = atomicAnd(c.sus32 + widx, ~(1u << pt.bit[0]));
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        if (u == 1 && n <= 32u) break;                             // warp-uniform
+        const uint32_t ty = pt.item[u] >> 16, tx = (pt.item[u] >> 3) & 0x1FFFu, d = pt.item[u] & 7u;
+        const uint32_t cell = ty * c.W + tx;
+        pt.bit[u] = ((ty & 3u) << 3) | (tx & 7u);
+        const uint32_t widx = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
+        uint32_t c3 = cell * kM0;
+        uint32_t c2 = __umulhi(cell, kM0) ^ (d >> 2) ^ ph.rk1[0];
+        uint32_t c0 = __umulhi(c2, kM1) ^ ph.x1;
+        uint32_t c1 = c2 * kM1;
+        c2 = ph.y1 ^ c3;
+        c3 = ph.a1l;
+#pragma unroll
+        for (int r = 2; r < 10; ++r) {
+            const uint64_t a = (uint64_t)c0 * kM0;
+            const uint64_t b = (uint64_t)c2 * kM1;
+            const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ ph.rk0[r];
+            const uint32_t n2 = (uint32_t)(a >> 32) ^ c3 ^ ph.rk1[r];
+            c1 = (uint32_t)b; c3 = (uint32_t)a; c0 = n0; c2 = n2;
+        }
+        const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
+        const uint32_t rnd = (d & 2u) ? hi : lo;
+        if (fire_trial(rnd, T[u])) pt.old[u] = atomicAnd(c.sus32 + widx, ~(1u << pt.bit[u]));
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -553,10 +583,7 @@ fire_propagate_async_kernel(const prop_params prm)
 
     for (;;) {
         __syncthreads();
-        if (tid == 0) {
-            const unsigned int k = atomicAdd(prm.work_counter, 1u);
-            s_sim = (k < (unsigned int)prm.S) ? (prm.order ? prm.order[k] : k) : 0xFFFFFFFFu;
-        }
+        if (tid == 0) s_sim = next_simulation(prm);
         __syncthreads();
         const uint32_t s = s_sim;
         if (s == 0xFFFFFFFFu) break;
@@ -604,7 +631,7 @@ fire_propagate_async_kernel(const prop_params prm)
             ph.a1l = r0c0 * kM0; ph.x1 = bl ^ ph.rk0[1]; ph.y1 = __umulhi(r0c0, kM0) ^ ph.rk1[1];
 
             uint32_t head = 0, fill = 0;                           // this warp's ring: entries [head, head + fill) mod kRingEntries
-            pending_trials<1> prev; bool have = false;
+            pending_trials<2> prev; bool have = false;
             const uint32_t nU = (c.nA + 31u) >> 5;
             for (uint32_t u = warp; u < nU; u += nwarps) {
                 // ---- one unit of 32 burning cells: window, thresholds, catch-up, trials appended to the ring
@@ -628,11 +655,12 @@ fire_propagate_async_kernel(const prop_params prm)
 
                 // while those loads are in flight: run the trials already in the ring
                 while (fill >= 32u) {
-                    pending_trials<1> cur;
-                    trials_issue_ring(c, ph, ring_addr, head, 32u, kRingEntries - 1u, cur);
-                    if (have) trials_resolve<1>(c, prev);
+                    const uint32_t n = fill >= 64u ? 64u : 32u;
+                    pending_trials<2> cur;
+                    trials_issue_ring(c, ph, ring_addr, head, n, kRingEntries - 1u, cur);
+                    if (have) trials_resolve<2>(c, prev);
                     prev = cur; have = true;
-                    head = (head + 32u) & (kRingEntries - 1u); fill -= 32u;
+                    head = (head + n) & (kRingEntries - 1u); fill -= n;
                 }
 
                 const uint32_t selr = ((by + 7u) & 7u) | (by << 4) | (((by + 1u) & 7u) << 8);
@@ -669,14 +697,14 @@ fire_propagate_async_kernel(const prop_params prm)
             }
             // ---- the rest of the ring, last unit possibly partial
             while (fill > 0u) {
-                const uint32_t n = fill < 32u ? fill : 32u;
-                pending_trials<1> cur;
+                const uint32_t n = fill < 64u ? fill : 64u;
+                pending_trials<2> cur;
                 trials_issue_ring(c, ph, ring_addr, head, n, kRingEntries - 1u, cur);
-                if (have) trials_resolve<1>(c, prev);
+                if (have) trials_resolve<2>(c, prev);
                 prev = cur; have = true;
                 head = (head + n) & (kRingEntries - 1u); fill -= n;
             }
-            if (have) trials_resolve<1>(c, prev);
+            if (have) trials_resolve<2>(c, prev);
             __syncthreads();
             ++t;
             if (s_over) { over = true; break; }
@@ -1029,7 +1057,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     prm.tiles = L->tiles; prm.plane_sel = L->status + S;
     prm.out_burned = out_burned; prm.out_steps = out_steps; prm.out_trials = (unsigned long long*)out_trials;
     prm.work_counter = L->work_counter; prm.rescue_list = L->status; prm.spill = L->spill;
-    prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.Tw = L->Tw; prm.Th = L->Th;
+    prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.Tw = L->Tw; prm.Th = L->Th; prm.num_sms = L->num_sms;
     prm.max_steps = max_steps;
 
     // ---- launch order: largest expected fires first (only matters when there are more simulations than resident CTAs)
@@ -1050,7 +1078,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         fire_init_tiles_kernel<<<dim3(chunks, (unsigned)(S * planes)), 256, 0, st>>>(L->burnable_tiles, L->tiles, nt);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
-    FIRE_CUDA_TRY(L, cudaMemsetAsync(L->work_counter, 0, 2 * sizeof(unsigned int), st));
+    FIRE_CUDA_TRY(L, cudaMemsetAsync(L->work_counter, 0, 4 * sizeof(unsigned int), st));
     if (async) FIRE_CUDA_TRY(L, cudaMemsetAsync(L->status + S, 0, (size_t)S * 4, st));
     void (*kernel)(const prop_params) = fire_propagate_kernel<1024, 1, 2, 4>;
     const int variant = L->kernel_variant;
@@ -1075,6 +1103,12 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     }
     if (smem + 1024 > 48 * 1024)                     // dynamic + static shared memory beyond the default limit
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    {   // ask for just the shared memory the resident CTAs need, so that the rest of the 228 KB stays L1 (the in-flight
+        // sector and tile loads of phase 1 live there)
+        int pct = (int)(((size_t)per_sm * (smem + 1024) * 100 + 228 * 1024 - 1) / (228 * 1024));
+        if (pct > 100) pct = 100;
+        FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct));
+    }
     const bool prof = L->prof_enabled && L->prof_count < 64;
     if (prof) FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count], st));
     kernel<<<grid, threads, smem, st>>>(prm);
