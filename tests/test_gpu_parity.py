@@ -327,3 +327,24 @@ def test_burned_area_distribution_ks(orc, request, cfg):
     report(request, gpu_mean_area=f"{ga.mean():.1f}", oracle_mean_area=f"{oa.mean():.1f}", ks_p=f"{ks.pvalue:.3f}")
     assert ks.pvalue > 0.01
     L.close()
+
+
+# ---------------------------------------------------------------------------------- search loop on top of the batch API (f1)
+def test_genetic_algorithm_drives_the_batch_api(request):
+    """PAPER.md App. B on config 1: calibrating against a reference burn simulated from a known vector, the GA's best
+    Eq. 2 fitness improves on the best of the random initial population and ends well below the no-information level."""
+    from paper_1701_03549_b200 import search
+    w = wl.load_workload(1)
+    L = gh.make_landscape(w.landscape)
+    gh.upload(L, w.ref_beta[None, :])
+    ref = gh.simulate(L, [w.ref_ignition], [0], [w.ref_seed], sim_ids=np.zeros(1, np.int32), keep_device=True)["burned"][0]
+    ev = search.Evaluator(L, ref, tuple(int(v) for v in w.ref_ignition), replicates=4, metric=0, seed=7)
+    lo = np.array([-6.0, -1.0, -0.5, 0.0, 0.0]); hi = np.array([2.0, 0.0, 0.5, 2.0, 1.5])
+    best, fit, hist = search.genetic_algorithm(ev, lo, hi, pop_size=64, generations=12, n_elite=2, seed=11)
+    report(request, first_generation_best=f"{hist[0][1]:.3f}", last_generation_best=f"{hist[-1][1]:.3f}", best=f"{fit:.3f}",
+           generations=len(hist), simulations=64 * 4 * 12)
+    assert fit <= hist[0][1] and fit < 0.6 and np.isfinite(fit)
+    assert ev.calls == 12 and (best >= lo).all() and (best <= hi).all()
+    _, fits = search.monte_carlo(ev, lo, hi, n_samples=256, batch=128, seed=12)
+    assert np.isfinite(fits[0]) and fits[0] < 1.0                       # App. C: brute force finds something better than "nothing burns"
+    L.close()
