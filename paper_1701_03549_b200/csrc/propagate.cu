@@ -147,7 +147,7 @@ struct step_ctx {
 
 // Phase 1 for K units of 32 burning cells (units u0, u0 + ustride, ...; all of them exist: u * 32 < nA).
 // Lanes past the end of the list re-read the last entry and contribute nothing.
-template <int K, bool kPartial>   // kPartial: units past the end of the frontier are skipped (warp-uniform guards)
+template <int K>
 __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, uint32_t ustride)
 {
     uint32_t e[K], win[K];
@@ -158,11 +158,6 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
     for (int k = 0; k < K; ++k) {
         uint32_t i = (u0 + (uint32_t)k * ustride) * 32u + c.lane;
         live[k] = i < c.nA;
-        if (kPartial && k > 0 && (u0 + (uint32_t)k * ustride) * 32u >= c.nA) {      // no such unit
-            e[k] = 0u; tc[k] = 0ull; th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
-            Ta[k] = make_uint4(0u, 0u, 0u, 0u); Tb[k] = make_uint4(0u, 0u, 0u, 0u);
-            continue;
-        }
         i = live[k] ? i : c.nA - 1u;
         e[k] = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.Ac_g + (i - c.capA_s));
         const uint32_t x = e[k] & 0xFFFFu, y = e[k] >> 16;
@@ -182,7 +177,6 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
     uint32_t cnt = 0;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
-        if (kPartial && k > 0 && (u0 + (uint32_t)k * ustride) * 32u >= c.nA) { win[k] = 0u; continue; }
         const uint32_t bx = e[k] & 7u, by = (e[k] >> 16) & 7u;
         // rows y-1, y, y+1 of the cell's tile column (w3c) and of the horizontally adjacent one (w3h), one per byte
         const uint32_t selr = ((by + 7u) & 7u) | (by << 4) | (((by + 1u) & 7u) << 8);
@@ -218,7 +212,6 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         if (w & (1u << (bit))) sts64(qa + 8u * __popc(w & ((1u << (bit)) - 1u)), base + item_delta(d), (Tv));
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            if (kPartial && k > 0 && (u0 + (uint32_t)k * ustride) * 32u >= c.nA) continue;
             const uint32_t w = win[k];
             const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
             const uint32_t qa = c.qs_addr + 8u * pos;
@@ -259,11 +252,12 @@ struct philox_step {
 // that the caller can overlap the atomics of one pass with the arithmetic of the next:
 //   trials_issue  : queue reads -> Philox -> compare -> atomicAnd on the susceptible plane (results left pending)
 //   trials_resolve: the lane whose atomic saw the bit still set owns the new burning cell -> next frontier
-template <int K> struct pending_trials { uint32_t item[K], bit[K], old[K]; };
+constexpr int kMaxInFlight = 4;
+struct pending_trials { uint32_t item[kMaxInFlight], bit[kMaxInFlight], old[kMaxInFlight]; };   // the first K entries are used
 
-template <int K, bool kPartial>   // kPartial: units past the end of the queue are skipped (warp-uniform guards)
+template <int K>
 __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_step& ph, uint32_t u0, uint32_t ustride,
-                                             pending_trials<K>& pt)
+                                             pending_trials& pt)
 {
     uint32_t T[K];
     const bool q_shared = (u0 + (uint32_t)(K - 1) * ustride + 1u) * 32u <= c.capQ_s;      // warp-uniform
@@ -278,7 +272,6 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
     }
 #pragma unroll
     for (int u = 0; u < K; ++u) {
-        if (kPartial && u > 0 && (u0 + (uint32_t)u * ustride) * 32u >= c.nQ) { pt.bit[u] = 0u; pt.old[u] = 0u; continue; }
         const uint32_t ty = pt.item[u] >> 16, tx = (pt.item[u] >> 3) & 0x1FFFu, d = pt.item[u] & 7u;
         const uint32_t cell = ty * c.W + tx;
         pt.bit[u] = ((ty & 3u) << 3) | (tx & 7u);
@@ -291,8 +284,11 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
         uint32_t c1 = c2 * kM1;
         c2 = ph.y1 ^ c3;
         c3 = ph.a1l;
+#ifndef FIRE_EXP_ROUNDS           // timing experiments only (wrong random numbers): fewer Philox rounds
+#define FIRE_EXP_ROUNDS 10
+#endif
 #pragma unroll
-        for (int r = 2; r < 10; ++r) {
+        for (int r = 2; r < FIRE_EXP_ROUNDS; ++r) {
             const uint64_t a = (uint64_t)c0 * kM0;
             const uint64_t b = (uint64_t)c2 * kM1;
             const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ ph.rk0[r];
@@ -312,7 +308,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
 }
 
 template <int K>
-__device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_trials<K>& pt)
+__device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_trials& pt)
 {
     uint32_t fresh_mask[K];
     uint32_t n_fresh = 0;
@@ -346,6 +342,26 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
             abase += __popc(fresh_mask[u]);
         }
     }
+}
+
+// A pass of exactly k units (1 <= k <= KMAX), k warp-uniform: one specialised body per k, so that the last pass of a
+// warp executes no code for units that do not exist.
+template <int KMAX>
+__device__ __forceinline__ void trials_issue_k(const step_ctx& c, const philox_step& ph, uint32_t u0, uint32_t ustride, int k,
+                                               pending_trials& pt)
+{
+    if (KMAX >= 4 && k == 4) trials_issue<4>(c, ph, u0, ustride, pt);
+    else if (KMAX >= 3 && k == 3) trials_issue<3>(c, ph, u0, ustride, pt);
+    else if (KMAX >= 2 && k == 2) trials_issue<2>(c, ph, u0, ustride, pt);
+    else trials_issue<1>(c, ph, u0, ustride, pt);
+}
+template <int KMAX>
+__device__ __forceinline__ void trials_resolve_k(const step_ctx& c, int k, const pending_trials& pt)
+{
+    if (KMAX >= 4 && k == 4) trials_resolve<4>(c, pt);
+    else if (KMAX >= 3 && k == 3) trials_resolve<3>(c, pt);
+    else if (KMAX >= 2 && k == 2) trials_resolve<2>(c, pt);
+    else if (k == 1) trials_resolve<1>(c, pt);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -431,8 +447,8 @@ fire_propagate_kernel(const prop_params prm)
                 const uint32_t nU = (c.nA + 31u) >> 5;
                 uint32_t u = warp;
                 for (; u + (uint32_t)(kCellsInFlight - 1) * nwarps < nU; u += nwarps * kCellsInFlight)
-                    my_trials += cells_pass<kCellsInFlight, false>(c, u, nwarps);
-                if (u < nU) my_trials += cells_pass<kCellsInFlight, true>(c, u, nwarps);
+                    my_trials += cells_pass<kCellsInFlight>(c, u, nwarps);
+                for (; u < nU; u += nwarps) my_trials += cells_pass<1>(c, u, nwarps);
             }
             __syncthreads();
             c.nQ = s_cntQ[par];
@@ -457,24 +473,21 @@ fire_propagate_kernel(const prop_params prm)
                 ph.y1 = __umulhi(r0c0, kM0) ^ ph.rk1[1];
                 const uint32_t nU = (c.nQ + 31u) >> 5;
                 uint32_t u = warp;
-                // passes of kTrialsInFlight units, software-pipelined: the atomics of a pass are resolved after the
-                // arithmetic of the next pass has been issued; the last pass of a warp may be partial
+                // passes of up to kTrialsInFlight units, software-pipelined: the atomics of a pass are resolved after the
+                // arithmetic of the next pass has been issued; the last pass of a warp has exactly the units that are left
                 {
-                    pending_trials<kTrialsInFlight> prev;
-                    bool have = false;
-                    for (; u + (uint32_t)(kTrialsInFlight - 1) * nwarps < nU; u += nwarps * kTrialsInFlight) {
-                        pending_trials<kTrialsInFlight> cur;
-                        trials_issue<kTrialsInFlight, false>(c, ph, u, nwarps, cur);
-                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
-                        prev = cur; have = true;
+                    pending_trials prev;
+                    int prev_k = 0;
+                    uint32_t left = (nU > u) ? (nU - u + nwarps - 1u) / nwarps : 0u;      // units of this warp
+                    while (left > 0u) {
+                        const int k = left >= (uint32_t)kTrialsInFlight ? kTrialsInFlight : (int)left;
+                        pending_trials cur;
+                        trials_issue_k<kTrialsInFlight>(c, ph, u, nwarps, k, cur);
+                        trials_resolve_k<kTrialsInFlight>(c, prev_k, prev);
+                        prev = cur; prev_k = k;
+                        u += nwarps * (uint32_t)k; left -= (uint32_t)k;
                     }
-                    if (u < nU) {
-                        pending_trials<kTrialsInFlight> cur;
-                        trials_issue<kTrialsInFlight, true>(c, ph, u, nwarps, cur);
-                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
-                        prev = cur; have = true;
-                    }
-                    if (have) trials_resolve<kTrialsInFlight>(c, prev);
+                    trials_resolve_k<kTrialsInFlight>(c, prev_k, prev);
                 }
             }
             __syncthreads();
@@ -505,7 +518,7 @@ fire_propagate_kernel(const prop_params prm)
 // The same first half for trials taken from a warp's own ring buffer (asynchronous-warp kernel): n <= 64 entries at `head`,
 // as two interleaved units of 32 (the second one is skipped when n <= 32).
 __device__ __forceinline__ void trials_issue_ring(const step_ctx& c, const philox_step& ph, uint32_t ring_addr, uint32_t head,
-                                                  uint32_t n, uint32_t ring_mask, pending_trials<2>& pt)
+                                                  uint32_t n, uint32_t ring_mask, pending_trials& pt)
 {
     uint32_t T[2];
 #pragma unroll
@@ -631,7 +644,7 @@ fire_propagate_async_kernel(const prop_params prm)
             ph.a1l = r0c0 * kM0; ph.x1 = bl ^ ph.rk0[1]; ph.y1 = __umulhi(r0c0, kM0) ^ ph.rk1[1];
 
             uint32_t head = 0, fill = 0;                           // this warp's ring: entries [head, head + fill) mod kRingEntries
-            pending_trials<2> prev; bool have = false;
+            pending_trials prev; bool have = false;
             const uint32_t nU = (c.nA + 31u) >> 5;
             for (uint32_t u = warp; u < nU; u += nwarps) {
                 // ---- one unit of 32 burning cells: window, thresholds, catch-up, trials appended to the ring
@@ -656,7 +669,7 @@ fire_propagate_async_kernel(const prop_params prm)
                 // while those loads are in flight: run the trials already in the ring
                 while (fill >= 32u) {
                     const uint32_t n = fill >= 64u ? 64u : 32u;
-                    pending_trials<2> cur;
+                    pending_trials cur;
                     trials_issue_ring(c, ph, ring_addr, head, n, kRingEntries - 1u, cur);
                     if (have) trials_resolve<2>(c, prev);
                     prev = cur; have = true;
@@ -698,7 +711,7 @@ fire_propagate_async_kernel(const prop_params prm)
             // ---- the rest of the ring, last unit possibly partial
             while (fill > 0u) {
                 const uint32_t n = fill < 64u ? fill : 64u;
-                pending_trials<2> cur;
+                pending_trials cur;
                 trials_issue_ring(c, ph, ring_addr, head, n, kRingEntries - 1u, cur);
                 if (have) trials_resolve<2>(c, prev);
                 prev = cur; have = true;
@@ -1088,6 +1101,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         kernel = variant == 1 ? fire_propagate_kernel<256, 6, 1, 2> : (variant == 2 ? fire_propagate_kernel<256, 6, 1, 4> : fire_propagate_kernel<256, 6, 2, 4>);
     else if (threads <= 256 && per_sm == 5)
         kernel = variant == 1 ? fire_propagate_kernel<256, 5, 1, 2> : (variant == 2 ? fire_propagate_kernel<256, 5, 1, 4> : fire_propagate_kernel<256, 5, 2, 4>);
+    else if (threads <= 256 && per_sm == 3) kernel = fire_propagate_kernel<256, 3, 2, 4>;
     else if (threads <= 256)
         kernel = variant == 2 ? fire_propagate_kernel<256, 4, 1, 4> : fire_propagate_kernel<256, 4, 2, 4>;
     else if (threads <= 512 && per_sm >= 4) kernel = variant == 1 ? fire_propagate_kernel<512, 4, 1, 1> : fire_propagate_kernel<512, 4, 1, 2>;
