@@ -64,12 +64,13 @@ fire_fitness_counts_kernel(const uint32_t* __restrict__ reference, const uint32_
     }
 }
 
-// #A of the reference map, one CTA.
+// #A of the reference map: grid-stride popcount, one integer atomic per CTA (*out zeroed before the launch).
 __global__ void __launch_bounds__(256)
 fire_reference_area_kernel(const uint32_t* __restrict__ reference, size_t nw, uint32_t* __restrict__ out)
 {
     uint32_t n = 0;
-    for (size_t i = threadIdx.x; i < nw; i += blockDim.x) n += __popc(__ldg(reference + i));
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nw; i += (size_t)gridDim.x * blockDim.x)
+        n += __popc(__ldg(reference + i));
     n = warp_sum(n);
     __shared__ uint32_t sh[8];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -78,7 +79,7 @@ fire_reference_area_kernel(const uint32_t* __restrict__ reference, size_t nw, ui
     if (threadIdx.x == 0) {
         uint32_t t = 0;
         for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += sh[w];
-        *out = t;
+        if (t) atomicAdd(out, t);
     }
 }
 
@@ -155,7 +156,12 @@ extern "C" int fire_fitness(fire_landscape* L, const uint32_t* reference, const 
     if ((size_t)words_per_cta > nw) words_per_cta = (uint32_t)((nw + 3) & ~(size_t)3);
     const unsigned chunks = (unsigned)((nw + words_per_cta - 1) / words_per_cta);
     FIRE_CUDA_TRY(L, cudaMemsetAsync(counts, 0, (size_t)S * 8, st));
-    fire_reference_area_kernel<<<1, 256, 0, st>>>(reference, nw, L->ref_area);
+    FIRE_CUDA_TRY(L, cudaMemsetAsync(L->ref_area, 0, sizeof(uint32_t), st));
+    {
+        unsigned ctas = (unsigned)((nw + 256 * 4 - 1) / (256 * 4));
+        if (ctas > 256) ctas = 256;
+        fire_reference_area_kernel<<<ctas, 256, 0, st>>>(reference, nw, L->ref_area);
+    }
     for (int s0 = 0; s0 < S; s0 += 65535) {                    // gridDim.y limit
         const int ns = (S - s0 < 65535) ? S - s0 : 65535;
         fire_fitness_counts_kernel<<<dim3(chunks, (unsigned)ns), 256, 0, st>>>(reference, burned + (size_t)s0 * nw, nw,

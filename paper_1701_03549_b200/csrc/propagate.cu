@@ -991,11 +991,13 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     cudaStream_t st = (cudaStream_t)stream;
 
     // ---- geometry and list capacities
-    // default: 1024 threads per SM, as 4 CTAs of 256 threads when there are enough simulations to fill them,
+    // default: 4 CTAs of 256 threads per SM when there are enough simulations to fill them (16 CTAs of 128 threads with the
+    // 32-register instantiation for very large batches on small lattices, whose fronts are a few dozen cells: config 4),
     // else fewer and wider CTAs so that a small batch of large fires still uses whole SMs
     int threads = L->threads_per_cta, per_sm = L->ctas_per_sm;
     if (threads == 0 && per_sm == 0) {
-        if ((long long)S >= 4ll * L->num_sms) { threads = 256; per_sm = 4; }
+        if ((long long)S >= 16ll * L->num_sms && L->cells <= (size_t)512 * 512) { threads = 128; per_sm = 16; }   // small lattice = short fronts
+        else if ((long long)S >= 4ll * L->num_sms) { threads = 256; per_sm = 4; }
         else if ((long long)S >= 2ll * L->num_sms) { threads = 512; per_sm = 2; }
         else { threads = 1024; per_sm = 1; }
     } else {
@@ -1004,7 +1006,12 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     }
     const int grid = (int)((long long)S < (long long)L->num_sms * per_sm ? S : L->num_sms * per_sm);
     prop_params prm;
-    uint32_t capA_s = L->list_shared ? (uint32_t)L->list_shared : 1536u;
+    uint32_t capA_s = 1536u;                                   // 24 B of shared memory per entry (two lists + 2 queue slots)
+    {
+        const uint32_t fit = (uint32_t)((180u * 1024u) / ((uint32_t)per_sm * 24u)) & ~127u;
+        if (capA_s > fit) capA_s = fit < 128u ? 128u : fit;
+    }
+    if (L->list_shared) capA_s = (uint32_t)L->list_shared;
     uint32_t capA = L->list_capacity ? (uint32_t)L->list_capacity : 0u;
     if (capA == 0) {
         // generous: a BFS level set of an open W x H lattice has at most 2(W+H) cells
