@@ -109,13 +109,6 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr)
     uint32_t v; asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
 }
 
-// List / queue slots beyond the shared-memory part (rare: only very long fronts get here).
-__device__ __noinline__ void spill_put_q(uint32_t qs_addr, uint2* Qg, uint32_t capQ_s, uint32_t q, uint32_t item, uint32_t T)
-{
-    if (q < capQ_s) sts64(qs_addr + 8u * q, item, T); else __stcg(Qg + (q - capQ_s), make_uint2(item, T));
-}
-
-
 // Next simulation for this CTA, or 0xFFFFFFFF: batch order, or the order written by fire_order_kernel (largest expected
 // fires first).  (Tried and dropped: CTAs of odd waves taking from the tail of the order, so that an SM hosts large and
 // small fires side by side -- the large fires do get faster, 23.3 -> 21.5 ms, but the medium ones then start late and the
@@ -284,11 +277,8 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
         uint32_t c1 = c2 * kM1;
         c2 = ph.y1 ^ c3;
         c3 = ph.a1l;
-#ifndef FIRE_EXP_ROUNDS           // timing experiments only (wrong random numbers): fewer Philox rounds
-#define FIRE_EXP_ROUNDS 10
-#endif
 #pragma unroll
-        for (int r = 2; r < FIRE_EXP_ROUNDS; ++r) {
+        for (int r = 2; r < 10; ++r) {
             const uint64_t a = (uint64_t)c0 * kM0;
             const uint64_t b = (uint64_t)c2 * kM1;
             const uint32_t n0 = (uint32_t)(b >> 32) ^ c1 ^ ph.rk0[r];
@@ -463,9 +453,6 @@ fire_propagate_kernel(const prop_params prm)
                 for (int r = 0; r < 10; ++r) {
                     ph.rk0[r] = key_lo + (uint32_t)r * kW0;
                     ph.rk1[r] = key_hi + (uint32_t)r * kW1;
-#ifdef FIRE_KEYS_IN_VECTOR_REGS
-                    asm volatile("" : "+r"(ph.rk0[r]), "+r"(ph.rk1[r]));
-#endif
                 }
                 const uint32_t r0c0 = bh ^ t ^ ph.rk0[0];                          // c0 after round 0
                 ph.a1l = r0c0 * kM0;                                               // round 1: c0 * M0
