@@ -378,6 +378,15 @@ def run_ours(args) -> None:
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms, "launches_timed": len(prop_ms),
                 "share_of_step": k_ms / ms_per_step,
                 "philox_calls_per_s": golden["totals"]["trials"] / (k_ms * 1e-3)}
+    # second ceiling: the kernel is issue-bound, not HBM-bound.  Algorithmic integer work = one
+    # Philox4x32-10 call per trial = 20 wide multiplies + 20 three-input xors = 40 lane operations; peak = SMs x 4 schedulers
+    # x 32 lanes x max SM clock, one instruction per scheduler per clock.
+    sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+    sm_clock_hz = 1e6 * float((clocks or {}).get("sm_max_mhz") or 1965.0)
+    alu_peak = sm_count * 4 * 32 * sm_clock_hz
+    alu_ach = 40.0 * golden["totals"]["trials"] / (k_ms * 1e-3)
+    roofline["alu"] = {"bound": "alu", "achieved": alu_ach / 1e12, "peak": alu_peak / 1e12, "unit": "Tera lane-ops/s",
+                       "frac": alu_ach / alu_peak, "note": "40 lane-ops per trial (Philox4x32-10) / issue peak"}
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample of the same workload
     cpu = None
