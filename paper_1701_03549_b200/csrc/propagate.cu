@@ -58,11 +58,12 @@ __device__ __forceinline__ uint32_t lanemask_lt()
     uint32_t m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m;
 }
 
-// Frontier entry: (y << 16) | x.  Trial item: (ty << 16) | (tx << 3) | d  (x, y < 8192).
+// Frontier entry: (y << 16) | x.  Trial item: (ty << 16) | (d << 13) | tx  (x, y < 8192): the frontier entry of the target
+// with the direction in the three spare bits, so that neither side shifts coordinates around.
 // Item of the trial "burning cell e spreads in direction d": item(e) + item_delta(d).
 __device__ __forceinline__ uint32_t item_delta(int d)
 {
-    return (uint32_t)(fire_dy(d) * 65536 + fire_dx(d) * 8 + d);
+    return (uint32_t)(fire_dy(d) * 65536 + fire_dx(d) + d * 8192);
 }
 
 // Threshold sector of a burning cell: read once, so keep it out of L1; the neighbouring sectors (the next
@@ -206,7 +207,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             const uint32_t w = win[k];
-            const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
+            const uint32_t base = e[k];
             const uint32_t qa = c.qs_addr + 8u * pos;
             FIRE_EMIT(0, 7, Tb[k].w)  FIRE_EMIT(1, 0, Ta[k].x)  FIRE_EMIT(2, 1, Ta[k].y)
             FIRE_EMIT(8, 6, Tb[k].z)  FIRE_EMIT(10, 2, Ta[k].z)
@@ -224,7 +225,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
 #pragma unroll
         for (int k = 0; k < K; ++k) {
             const uint32_t w = win[k];
-            const uint32_t base = ((e[k] & 0xFFFFu) << 3) | (e[k] & 0xFFFF0000u);
+            const uint32_t base = e[k];
             FIRE_EMIT(0, 7, Tb[k].w)  FIRE_EMIT(1, 0, Ta[k].x)  FIRE_EMIT(2, 1, Ta[k].y)
             FIRE_EMIT(8, 6, Tb[k].z)  FIRE_EMIT(10, 2, Ta[k].z)
             FIRE_EMIT(16, 5, Tb[k].y) FIRE_EMIT(17, 4, Tb[k].x) FIRE_EMIT(18, 3, Ta[k].w)
@@ -265,7 +266,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
     }
 #pragma unroll
     for (int u = 0; u < K; ++u) {
-        const uint32_t ty = pt.item[u] >> 16, tx = (pt.item[u] >> 3) & 0x1FFFu, d = pt.item[u] & 7u;
+        const uint32_t ty = pt.item[u] >> 16, tx = pt.item[u] & 0x1FFFu, d = (pt.item[u] >> 13) & 7u;
         const uint32_t cell = ty * c.W + tx;
         pt.bit[u] = ((ty & 3u) << 3) | (tx & 7u);
         const uint32_t widx = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
@@ -314,7 +315,7 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
     if (abase + n_fresh <= c.capA_s) {                             // warp-uniform: all new cells go to shared memory
 #pragma unroll
         for (int u = 0; u < K; ++u) {
-            const uint32_t en = (pt.item[u] & 0xFFFF0000u) | ((pt.item[u] >> 3) & 0x1FFFu);
+            const uint32_t en = pt.item[u] & 0xFFFF1FFFu;
             const uint32_t a = c.an_addr + 4u * (abase + __popc(fresh_mask[u] & c.lt));
             if (fresh_mask[u] & (1u << c.lane)) sts32(a, en);
             abase += __popc(fresh_mask[u]);
@@ -324,7 +325,7 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
         for (int u = 0; u < K; ++u) {
             if (fresh_mask[u] & (1u << c.lane)) {
                 const uint32_t pos = abase + __popc(fresh_mask[u] & c.lt);
-                const uint32_t en = (pt.item[u] & 0xFFFF0000u) | ((pt.item[u] >> 3) & 0x1FFFu);
+                const uint32_t en = pt.item[u] & 0xFFFF1FFFu;
                 if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, en);
                 else if (pos < c.capA) __stcg(c.An_g + (pos - c.capA_s), en);
                 else sts32(c.over, 1u);
@@ -519,7 +520,7 @@ __device__ __forceinline__ void trials_issue_ring(const step_ctx& c, const philo
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
         if (u == 1 && n <= 32u) break;                             // warp-uniform
-        const uint32_t ty = pt.item[u] >> 16, tx = (pt.item[u] >> 3) & 0x1FFFu, d = pt.item[u] & 7u;
+        const uint32_t ty = pt.item[u] >> 16, tx = pt.item[u] & 0x1FFFu, d = (pt.item[u] >> 13) & 7u;
         const uint32_t cell = ty * c.W + tx;
         pt.bit[u] = ((ty & 3u) << 3) | (tx & 7u);
         const uint32_t widx = (((ty >> 3) * c.Tw + (tx >> 3)) << 1) | ((ty >> 2) & 1u);
@@ -685,7 +686,7 @@ fire_propagate_async_kernel(const prop_params prm)
                 const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
                 my_trials += cnt;
                 const uint32_t pos = head + fill + incl - cnt;
-                const uint32_t base = ((e & 0xFFFFu) << 3) | (e & 0xFFFF0000u);
+                const uint32_t base = e;
 #define FIRE_EMIT(bit, d, Tv) \
                 if (w & (1u << (bit))) sts64(ring_addr + 8u * ((pos + __popc(w & ((1u << (bit)) - 1u))) & (kRingEntries - 1u)), base + item_delta(d), (Tv));
                 FIRE_EMIT(0, 7, Tb.w)  FIRE_EMIT(1, 0, Ta.x)  FIRE_EMIT(2, 1, Ta.y)
