@@ -254,15 +254,26 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
                                              pending_trials& pt)
 {
     uint32_t T[K];
-    const bool q_shared = (u0 + (uint32_t)(K - 1) * ustride + 1u) * 32u <= c.capQ_s;      // warp-uniform
+    if ((u0 + (uint32_t)(K - 1) * ustride + 1u) * 32u <= c.capQ_s) {                       // warp-uniform: all in shared memory
 #pragma unroll
-    for (int u = 0; u < K; ++u) {
-        uint32_t j = (u0 + (uint32_t)u * ustride) * 32u + c.lane;     // (clamped below: a unit past the end re-reads the last entry)
-        const bool live = j < c.nQ;
-        j = live ? j : c.nQ - 1u;
-        const uint2 it = (q_shared || j < c.capQ_s) ? lds64(c.qs_addr + 8u * j) : __ldcg(c.Qg + (j - c.capQ_s));
-        pt.item[u] = it.x;
-        T[u] = live ? it.y : 0u;                                   // T = 0 never succeeds
+        for (int u = 0; u < K; ++u) {
+            uint32_t j = (u0 + (uint32_t)u * ustride) * 32u + c.lane;
+            const bool live = j < c.nQ;
+            j = live ? j : c.nQ - 1u;                              // a lane past the end re-reads the last entry
+            const uint2 it = lds64(c.qs_addr + 8u * j);
+            pt.item[u] = it.x;
+            T[u] = live ? it.y : 0u;                               // T = 0 never succeeds
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < K; ++u) {
+            uint32_t j = (u0 + (uint32_t)u * ustride) * 32u + c.lane;
+            const bool live = j < c.nQ;
+            j = live ? j : c.nQ - 1u;
+            const uint2 it = (j < c.capQ_s) ? lds64(c.qs_addr + 8u * j) : __ldcg(c.Qg + (j - c.capQ_s));
+            pt.item[u] = it.x;
+            T[u] = live ? it.y : 0u;
+        }
     }
 #pragma unroll
     for (int u = 0; u < K; ++u) {
@@ -378,6 +389,7 @@ fire_propagate_kernel(const prop_params prm)
 
     const int tid = threadIdx.x;
     const uint32_t warp = (uint32_t)tid >> 5, nwarps = blockDim.x >> 5;
+    const uint32_t inv_nwarps = 0xFFFFFFFFu / nwarps + 1u;      // floor(x / nwarps) = umulhi(x, inv) for every x < 2^32 / nwarps
 
     step_ctx c;
     c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th;
@@ -466,7 +478,7 @@ fire_propagate_kernel(const prop_params prm)
                 {
                     pending_trials prev;
                     int prev_k = 0;
-                    uint32_t left = (nU > u) ? (nU - u + nwarps - 1u) / nwarps : 0u;      // units of this warp
+                    uint32_t left = (nU > u) ? __umulhi(nU - u + nwarps - 1u, inv_nwarps) : 0u;      // units of this warp: ceil((nU - u) / nwarps)
                     while (left > 0u) {
                         const int k = left >= (uint32_t)kTrialsInFlight ? kTrialsInFlight : (int)left;
                         pending_trials cur;
