@@ -389,7 +389,8 @@ fire_propagate_kernel(const prop_params prm)
 
     const int tid = threadIdx.x;
     const uint32_t warp = (uint32_t)tid >> 5, nwarps = blockDim.x >> 5;
-    const uint32_t inv_nwarps = 0xFFFFFFFFu / nwarps + 1u;      // floor(x / nwarps) = umulhi(x, inv) for every x < 2^32 / nwarps
+    // floor(x / nwarps) = umulhi(x, inv) for every x < 2^32 / nwarps; 0 stands for nwarps = 1 (its reciprocal does not fit)
+    const uint32_t inv_nwarps = nwarps > 1u ? 0xFFFFFFFFu / nwarps + 1u : 0u;
 
     step_ctx c;
     c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th;
@@ -478,7 +479,7 @@ fire_propagate_kernel(const prop_params prm)
                 {
                     pending_trials prev;
                     int prev_k = 0;
-                    uint32_t left = (nU > u) ? __umulhi(nU - u + nwarps - 1u, inv_nwarps) : 0u;      // units of this warp: ceil((nU - u) / nwarps)
+                    uint32_t left = (nU > u) ? (inv_nwarps ? __umulhi(nU - u + nwarps - 1u, inv_nwarps) : nU - u) : 0u;      // units of this warp: ceil((nU - u) / nwarps)
                     while (left > 0u) {
                         const int k = left >= (uint32_t)kTrialsInFlight ? kTrialsInFlight : (int)left;
                         pending_trials cur;
