@@ -478,17 +478,22 @@ fire_propagate_kernel(const prop_params prm)
                 // arithmetic of the next pass has been issued; the last pass of a warp has exactly the units that are left
                 {
                     pending_trials prev;
-                    int prev_k = 0;
+                    bool have = false;
                     uint32_t left = (nU > u) ? (inv_nwarps ? __umulhi(nU - u + nwarps - 1u, inv_nwarps) : nU - u) : 0u;      // units of this warp: ceil((nU - u) / nwarps)
-                    while (left > 0u) {
-                        const int k = left >= (uint32_t)kTrialsInFlight ? kTrialsInFlight : (int)left;
+                    for (; left >= (uint32_t)kTrialsInFlight; left -= (uint32_t)kTrialsInFlight, u += nwarps * kTrialsInFlight) {
                         pending_trials cur;
-                        trials_issue_k<kTrialsInFlight>(c, ph, u, nwarps, k, cur);
-                        trials_resolve_k<kTrialsInFlight>(c, prev_k, prev);
-                        prev = cur; prev_k = k;
-                        u += nwarps * (uint32_t)k; left -= (uint32_t)k;
+                        trials_issue<kTrialsInFlight>(c, ph, u, nwarps, cur);
+                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
+                        prev = cur; have = true;
                     }
-                    trials_resolve_k<kTrialsInFlight>(c, prev_k, prev);
+                    if (left > 0u) {                               // the last, shorter pass: specialised by its exact size
+                        pending_trials cur;
+                        trials_issue_k<kTrialsInFlight>(c, ph, u, nwarps, (int)left, cur);
+                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
+                        trials_resolve_k<kTrialsInFlight>(c, (int)left, cur);
+                    } else if (have) {
+                        trials_resolve<kTrialsInFlight>(c, prev);
+                    }
                 }
             }
             __syncthreads();
