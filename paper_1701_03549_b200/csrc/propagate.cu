@@ -1132,7 +1132,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     {   // ask for just the shared memory the resident CTAs need, so that the rest of the 228 KB stays L1 (the in-flight
         // sector and tile loads of phase 1 live there)
-        int pct = (int)(((size_t)per_sm * (smem + 1024) * 100 + 228 * 1024 - 1) / (228 * 1024));
+        int pct = (int)(((size_t)per_sm * (smem + 1024 + 256) * 100 + 228 * 1024 - 1) / (228 * 1024));   // + 1 KiB reserved per CTA + static shared memory
         if (pct > 100) pct = 100;
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct));
     }
