@@ -66,20 +66,19 @@ __device__ __forceinline__ uint32_t item_delta(int d)
     return (uint32_t)(fire_dy(d) * 65536 + fire_dx(d) + d * 8192);
 }
 
-// Threshold sector of a burning cell (read-only path).  The table is read once per simulation, but the 128 B line around a
-// sector holds the sectors of the 3 neighbouring cells of the row, which the same CTA needs in the next steps as the front
-// moves on: letting the line live in L1 (and asking L2 to fetch all of it with the miss) beats bypassing L1
-// (4.23 against 4.62 ns per trial).
-__device__ __forceinline__ uint4 ldg_thr(const uint4* p)
+// Threshold sector of a burning cell: ONE 256-bit load (LDG.E.256, sm_100) through the read-only path.  The table is
+// read once per simulation, so the line need not stay in L1; L2 is asked to fetch the whole 128 B line with the miss, since
+// the 3 neighbouring cells of the row are what the front reaches next.
+struct thr_sector { uint4 a, b; };     // a = directions 0..3, b = directions 4..7
+__device__ __forceinline__ thr_sector ldg_thr(const uint4* p)
 {
-    uint4 v;
-#if defined(FIRE_THR_NO_L1)
-    asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
-#elif defined(FIRE_THR_L2_256)
-    asm volatile("ld.global.nc.L2::256B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    thr_sector v;
+#if defined(FIRE_THR_L1)
+    asm volatile("ld.global.nc.L2::128B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
 #else
-    asm volatile("ld.global.nc.L2::128B.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
 #endif
+                 : "=r"(v.a.x), "=r"(v.a.y), "=r"(v.a.z), "=r"(v.a.w), "=r"(v.b.x), "=r"(v.b.y), "=r"(v.b.z), "=r"(v.b.w) : "l"(p));
     return v;
 }
 
@@ -163,8 +162,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
         const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
         tc[k] = ldcg_u64(c.sus + tidx);
-        Ta[k] = ldg_thr(sp);
-        Tb[k] = ldg_thr(sp + 1);
+        { const thr_sector ts = ldg_thr(sp); Ta[k] = ts.a; Tb[k] = ts.b; }
         th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
         if (hoff) th[k] = ldcg_u64(c.sus + (tidx + hoff));
         if (voff) tv[k] = ldcg_u64(c.sus + (tidx + voff));
@@ -667,7 +665,8 @@ fire_propagate_async_kernel(const prop_params prm)
                 const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
                 const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
                 const uint64_t tc = ldcg_u64(c.sus + tidx);
-                const uint4 Ta = ldg_thr(sp), Tb = ldg_thr(sp + 1);
+                const thr_sector ts = ldg_thr(sp);
+                const uint4 Ta = ts.a, Tb = ts.b;
                 uint64_t th = 0ull, tv = 0ull, td = 0ull;
                 if (hoff) th = ldcg_u64(c.sus + (tidx + hoff));
                 if (voff) tv = ldcg_u64(c.sus + (tidx + voff));
