@@ -128,8 +128,11 @@ __device__ __forceinline__ uint32_t next_simulation(const prop_params& prm)
 struct step_ctx {
     // lattice / tables
     uint32_t W, Tw, Th;
-    const uint64_t* sus;          // susceptible plane of this simulation, tile layout
-    uint32_t* sus32;              // the same, as 8 x 4-cell half tiles (atomics)
+    // susceptible planes: the base is the kernel parameter (a constant-bank operand of the address arithmetic); a plane is a
+    // 32-bit tile offset from it, so no 64-bit pointer per simulation has to live in (or be rebuilt into) registers
+    const uint64_t* tiles;
+    uint32_t plane_r;             // tile offset of the plane this step READS
+    uint32_t plane_w;             // tile offset of the plane this step UPDATES (the same plane in the two-phase kernel)
     const uint4* thr4;            // threshold sectors of this simulation's parameter vector, 2 x uint4 per source cell
     // lists
     uint32_t qs_addr, ac_addr, an_addr;   // shared-window addresses: trial queue, current frontier, next frontier
@@ -161,12 +164,12 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         const int hoff = (bx == 0u && tx0 > 0u) ? -1 : ((bx == 7u && tx0 + 1u < c.Tw) ? 1 : 0);
         const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
         const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
-        tc[k] = ldcg_u64(c.sus + tidx);
+        tc[k] = ldcg_u64(c.tiles + (c.plane_r + tidx));
         { const thr_sector ts = ldg_thr(sp); Ta[k] = ts.a; Tb[k] = ts.b; }
         th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
-        if (hoff) th[k] = ldcg_u64(c.sus + (tidx + hoff));
-        if (voff) tv[k] = ldcg_u64(c.sus + (tidx + voff));
-        if (hoff && voff) td[k] = ldcg_u64(c.sus + (tidx + hoff + voff));
+        if (hoff) th[k] = ldcg_u64(c.tiles + (c.plane_r + tidx + hoff));
+        if (voff) tv[k] = ldcg_u64(c.tiles + (c.plane_r + tidx + voff));
+        if (hoff && voff) td[k] = ldcg_u64(c.tiles + (c.plane_r + tidx + hoff + voff));
     }
     uint32_t cnt = 0;
 #pragma unroll
@@ -301,7 +304,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
         const uint32_t rnd = (d & 2u) ? hi : lo;
         pt.old[u] = 0u;
         if (fire_trial(rnd, T[u])) {
-            pt.old[u] = atomicAnd(c.sus32 + widx, ~(1u << pt.bit[u]));
+            pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + ((c.plane_w << 1) + widx), ~(1u << pt.bit[u]));
 #ifdef FIRE_PREFETCH_THR
             asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)(cell * 2u)));
 #endif
@@ -393,7 +396,7 @@ fire_propagate_kernel(const prop_params prm)
     const uint32_t inv_nwarps = nwarps > 1u ? 0xFFFFFFFFu / nwarps + 1u : 0u;
 
     step_ctx c;
-    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th;
+    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles;
     c.qs_addr = qs_addr; c.capQ_s = prm.capQ_s; c.capA_s = prm.capA_s; c.capA = prm.capA;
     c.Qg = reinterpret_cast<uint2*>(prm.spill + (size_t)blockIdx.x * spill_per_cta);
     c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
@@ -414,8 +417,7 @@ fire_propagate_kernel(const prop_params prm)
         const int ix = prm.ignitions[2 * s], iy = prm.ignitions[2 * s + 1];
         const uint64_t seed = prm.seeds[s];
         const uint32_t sim = prm.sim_ids ? (uint32_t)prm.sim_ids[s] : s;
-        c.sus = prm.tiles + (size_t)s * c.Tw * c.Th;
-        c.sus32 = reinterpret_cast<uint32_t*>(prm.tiles + (size_t)s * c.Tw * c.Th);
+        c.plane_r = c.plane_w = s * (c.Tw * c.Th);             // the host checks that S * tiles fits 31 bits
         bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
         if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
         c.thr4 = reinterpret_cast<const uint4*>(prm.thr + (valid ? (size_t)p * c.W * prm.H * 8 : 0));
@@ -431,7 +433,7 @@ fire_propagate_kernel(const prop_params prm)
             if (valid) {
                 const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
                 if (prm.capA_s > 0) sts32(as_addr0, e0); else Ag0[0] = e0;
-                atomicAnd(c.sus32 + (((size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
+                atomicAnd(reinterpret_cast<uint32_t*>(prm.tiles) + (((size_t)c.plane_w + (size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
         }
         __syncthreads();
@@ -558,7 +560,7 @@ __device__ __forceinline__ void trials_issue_ring(const step_ctx& c, const philo
         }
         const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
         const uint32_t rnd = (d & 2u) ? hi : lo;
-        if (fire_trial(rnd, T[u])) pt.old[u] = atomicAnd(c.sus32 + widx, ~(1u << pt.bit[u]));
+        if (fire_trial(rnd, T[u])) pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + ((c.plane_w << 1) + widx), ~(1u << pt.bit[u]));
     }
 }
 
@@ -593,7 +595,7 @@ fire_propagate_async_kernel(const prop_params prm)
     __shared__ unsigned long long s_trials;
 
     step_ctx c;
-    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th;
+    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles;
     c.capA_s = prm.capA_s; c.capA = prm.capA; c.capQ_s = 0u; c.qs_addr = 0u; c.Qg = nullptr; c.cntQ = 0u; c.nQ = 0u;
     c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
     const uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]);
@@ -614,6 +616,7 @@ fire_propagate_async_kernel(const prop_params prm)
         const uint64_t seed = prm.seeds[s];
         const uint32_t sim = prm.sim_ids ? (uint32_t)prm.sim_ids[s] : s;
         uint64_t* const plane0 = prm.tiles + (size_t)s * 2 * nt;
+        const uint32_t plane0_t = s * 2u * (uint32_t)nt;
         bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
         if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
         c.thr4 = reinterpret_cast<const uint4*>(prm.thr + (valid ? (size_t)p * c.W * prm.H * 8 : 0));
@@ -640,8 +643,8 @@ fire_propagate_async_kernel(const prop_params prm)
             c.Ac_g = par ? Ag1 : Ag0; c.An_g = par ? Ag0 : Ag1;
             c.cntA_next = cntA_addr + 4u * ((t + 1u) % 3u);
             if (tid == 0) s_cntA[(t + 2u) % 3u] = 0u;             // read last at the start of step t - 1, appended to in step t + 1
-            c.sus = plane0 + (size_t)par * nt;                                              // read plane
-            c.sus32 = reinterpret_cast<uint32_t*>(plane0 + (size_t)(par ^ 1u) * nt);        // written plane
+            c.plane_r = plane0_t + par * (uint32_t)nt;                                        // read plane
+            c.plane_w = plane0_t + (par ^ 1u) * (uint32_t)nt;                                 // written plane
 
             philox_step ph;
 #pragma unroll
@@ -664,14 +667,14 @@ fire_propagate_async_kernel(const prop_params prm)
                 const int hoff = (bx == 0u && tx0 > 0u) ? -1 : ((bx == 7u && tx0 + 1u < c.Tw) ? 1 : 0);
                 const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
                 const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
-                const uint64_t tc = ldcg_u64(c.sus + tidx);
+                const uint64_t tc = ldcg_u64(c.tiles + (c.plane_r + tidx));
                 const thr_sector ts = ldg_thr(sp);
                 const uint4 Ta = ts.a, Tb = ts.b;
                 uint64_t th = 0ull, tv = 0ull, td = 0ull;
-                if (hoff) th = ldcg_u64(c.sus + (tidx + hoff));
-                if (voff) tv = ldcg_u64(c.sus + (tidx + voff));
-                if (hoff && voff) td = ldcg_u64(c.sus + (tidx + hoff + voff));
-                if (live) atomicAnd(c.sus32 + ((tidx << 1) | ((y >> 2) & 1u)), ~(1u << (((y & 3u) << 3) | bx)));      // catch-up (no return: RED)
+                if (hoff) th = ldcg_u64(c.tiles + (c.plane_r + tidx + hoff));
+                if (voff) tv = ldcg_u64(c.tiles + (c.plane_r + tidx + voff));
+                if (hoff && voff) td = ldcg_u64(c.tiles + (c.plane_r + tidx + hoff + voff));
+                if (live) atomicAnd(reinterpret_cast<uint32_t*>(prm.tiles) + (((c.plane_w + tidx) << 1) | ((y >> 2) & 1u)), ~(1u << (((y & 3u) << 3) | bx)));      // catch-up (no return: RED)
 
                 // while those loads are in flight: run the trials already in the ring
                 while (fill >= 32u) {
@@ -1050,6 +1053,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     const size_t nw = (size_t)L->H * L->Ww;
     const size_t nt = (size_t)L->Tw * L->Th;
     const size_t rescue_bytes = nw * 4 * 2 * kRescueCtas;
+    if (nt * (size_t)S * 2 >= ((size_t)1 << 31)) return FIRE_EINVAL;   // planes are addressed by 32-bit tile offsets: split the batch
     const size_t tiles_bytes = nt * 8 * (size_t)S * 2;        // room for two planes per simulation
     if (L->status_capacity < (size_t)2 * S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes ||
         L->tiles_capacity < tiles_bytes || L->order_capacity < (size_t)S * 4 || L->burnable_tiles == nullptr) {
