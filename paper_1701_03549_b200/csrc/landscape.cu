@@ -267,6 +267,7 @@ extern "C" int fire_params_upload(fire_landscape* L, const float* beta, int32_t 
     if (L->sticky) return L->sticky;
     fire_device_guard g(L->device);
     if (!g.ok) return FIRE_ECUDA;
+    if ((size_t)P * L->cells >= ((size_t)1 << 32)) return FIRE_EINVAL;   // sectors are addressed by 32-bit indices (2^32 sectors = 137 GB)
     const size_t bytes = (size_t)P * L->cells * 32;
     if (L->thr_capacity < bytes) {
         // growing the table must not race with work still using the old one

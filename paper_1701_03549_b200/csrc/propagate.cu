@@ -133,7 +133,8 @@ struct step_ctx {
     const uint64_t* tiles;
     uint32_t plane_r;             // tile offset of the plane this step READS
     uint32_t plane_w;             // tile offset of the plane this step UPDATES (the same plane in the two-phase kernel)
-    const uint4* thr4;            // threshold sectors of this simulation's parameter vector, 2 x uint4 per source cell
+    const uint4* thr4;            // the threshold table (kernel parameter), 2 x uint4 per sector
+    uint32_t thr_sec;             // first sector of this simulation's parameter vector (a table that fits in HBM has < 2^32 sectors)
     // lists
     uint32_t qs_addr, ac_addr, an_addr;   // shared-window addresses: trial queue, current frontier, next frontier
     uint32_t capQ_s, capA_s, capA;
@@ -163,7 +164,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         const uint32_t tidx = ty0 * c.Tw + tx0;
         const int hoff = (bx == 0u && tx0 > 0u) ? -1 : ((bx == 7u && tx0 + 1u < c.Tw) ? 1 : 0);
         const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
-        const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
+        const uint4* const sp = c.thr4 + (size_t)(c.thr_sec + y * c.W + x) * 2;
         tc[k] = ldcg_u64(c.tiles + (c.plane_r + tidx));
         { const thr_sector ts = ldg_thr(sp); Ta[k] = ts.a; Tb[k] = ts.b; }
         th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
@@ -306,7 +307,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
         if (fire_trial(rnd, T[u])) {
             pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + ((c.plane_w << 1) + widx), ~(1u << pt.bit[u]));
 #ifdef FIRE_PREFETCH_THR
-            asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)(cell * 2u)));
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)(c.thr_sec + cell) * 2));
 #endif
         }
     }
@@ -396,7 +397,7 @@ fire_propagate_kernel(const prop_params prm)
     const uint32_t inv_nwarps = nwarps > 1u ? 0xFFFFFFFFu / nwarps + 1u : 0u;
 
     step_ctx c;
-    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles;
+    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles; c.thr4 = reinterpret_cast<const uint4*>(prm.thr);
     c.qs_addr = qs_addr; c.capQ_s = prm.capQ_s; c.capA_s = prm.capA_s; c.capA = prm.capA;
     c.Qg = reinterpret_cast<uint2*>(prm.spill + (size_t)blockIdx.x * spill_per_cta);
     c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
@@ -420,7 +421,7 @@ fire_propagate_kernel(const prop_params prm)
         c.plane_r = c.plane_w = s * (c.Tw * c.Th);             // the host checks that S * tiles fits 31 bits
         bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
         if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
-        c.thr4 = reinterpret_cast<const uint4*>(prm.thr + (valid ? (size_t)p * c.W * prm.H * 8 : 0));
+        c.thr_sec = valid ? (uint32_t)p * (c.W * (uint32_t)prm.H) : 0u;
         // the key is the same in every lane: a warp reduction leaves it in a UNIFORM register, and so are the round keys
         // derived from it (they then cost no per-thread registers)
         const uint32_t key_lo = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)seed), key_hi = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)(seed >> 32));
@@ -595,7 +596,7 @@ fire_propagate_async_kernel(const prop_params prm)
     __shared__ unsigned long long s_trials;
 
     step_ctx c;
-    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles;
+    c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles; c.thr4 = reinterpret_cast<const uint4*>(prm.thr);
     c.capA_s = prm.capA_s; c.capA = prm.capA; c.capQ_s = 0u; c.qs_addr = 0u; c.Qg = nullptr; c.cntQ = 0u; c.nQ = 0u;
     c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
     const uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]);
@@ -619,7 +620,7 @@ fire_propagate_async_kernel(const prop_params prm)
         const uint32_t plane0_t = s * 2u * (uint32_t)nt;
         bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
         if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
-        c.thr4 = reinterpret_cast<const uint4*>(prm.thr + (valid ? (size_t)p * c.W * prm.H * 8 : 0));
+        c.thr_sec = valid ? (uint32_t)p * (c.W * (uint32_t)prm.H) : 0u;
         const uint32_t key_lo = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)seed), key_hi = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)(seed >> 32));
         const uint32_t bh = __umulhi(sim, kM1), bl = sim * kM1;
 
@@ -666,7 +667,7 @@ fire_propagate_async_kernel(const prop_params prm)
                 const uint32_t tidx = ty0 * c.Tw + tx0;
                 const int hoff = (bx == 0u && tx0 > 0u) ? -1 : ((bx == 7u && tx0 + 1u < c.Tw) ? 1 : 0);
                 const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
-                const uint4* const sp = c.thr4 + (size_t)((y * c.W + x) * 2u);
+                const uint4* const sp = c.thr4 + (size_t)(c.thr_sec + y * c.W + x) * 2;
                 const uint64_t tc = ldcg_u64(c.tiles + (c.plane_r + tidx));
                 const thr_sector ts = ldg_thr(sp);
                 const uint4 Ta = ts.a, Tb = ts.b;
