@@ -138,7 +138,8 @@ struct step_ctx {
     // lists
     uint32_t qs_addr, ac_addr, an_addr;   // shared-window addresses: trial queue, current frontier, next frontier
     uint32_t capQ_s, capA_s, capA;
-    uint2* Qg; const uint32_t* Ac_g; uint32_t* An_g;
+    uint32_t* spill;              // per-CTA global spill areas (kernel parameter) and 32-bit word offsets into it:
+    uint32_t qg_off, ac_off, an_off;   // trial queue (8 B entries), current frontier, next frontier beyond their shared-memory parts
     uint32_t cntQ, cntA_next, over;       // shared-window addresses of the queue counter, the next frontier's counter, the overflow flag
     uint32_t nA, nQ;
     uint32_t lane, lt;
@@ -158,7 +159,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         uint32_t i = (u0 + (uint32_t)k * ustride) * 32u + c.lane;
         live[k] = i < c.nA;
         i = live[k] ? i : c.nA - 1u;
-        e[k] = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.Ac_g + (i - c.capA_s));
+        e[k] = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.spill + (c.ac_off + (i - c.capA_s)));
         const uint32_t x = e[k] & 0xFFFFu, y = e[k] >> 16;
         const uint32_t tx0 = x >> 3, ty0 = y >> 3, bx = x & 7u, by = y & 7u;
         const uint32_t tidx = ty0 * c.Tw + tx0;
@@ -224,7 +225,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         if (w & (1u << (bit))) { \
             const uint32_t q = pos + __popc(w & ((1u << (bit)) - 1u)); \
             if (q < c.capQ_s) sts64(c.qs_addr + 8u * q, base + item_delta(d), (Tv)); \
-            else __stcg(c.Qg + (q - c.capQ_s), make_uint2(base + item_delta(d), (Tv))); \
+            else __stcg(reinterpret_cast<uint2*>(c.spill + c.qg_off) + (q - c.capQ_s), make_uint2(base + item_delta(d), (Tv))); \
         }
 #pragma unroll
         for (int k = 0; k < K; ++k) {
@@ -274,7 +275,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
             uint32_t j = (u0 + (uint32_t)u * ustride) * 32u + c.lane;
             const bool live = j < c.nQ;
             j = live ? j : c.nQ - 1u;
-            const uint2 it = (j < c.capQ_s) ? lds64(c.qs_addr + 8u * j) : __ldcg(c.Qg + (j - c.capQ_s));
+            const uint2 it = (j < c.capQ_s) ? lds64(c.qs_addr + 8u * j) : __ldcg(reinterpret_cast<const uint2*>(c.spill + c.qg_off) + (j - c.capQ_s));
             pt.item[u] = it.x;
             T[u] = live ? it.y : 0u;
         }
@@ -342,7 +343,7 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
                 const uint32_t pos = abase + __popc(fresh_mask[u] & c.lt);
                 const uint32_t en = pt.item[u] & 0xFFFF1FFFu;
                 if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, en);
-                else if (pos < c.capA) __stcg(c.An_g + (pos - c.capA_s), en);
+                else if (pos < c.capA) __stcg(c.spill + (c.an_off + (pos - c.capA_s)), en);
                 else sts32(c.over, 1u);
             }
             abase += __popc(fresh_mask[u]);
@@ -385,8 +386,9 @@ fire_propagate_kernel(const prop_params prm)
     asm volatile("" : "+r"(qs_addr));            // keep it in a register: ptxas would otherwise rebuild the window address at every use
     const uint32_t as_addr0 = qs_addr + 8u * prm.capQ_s, as_addr1 = as_addr0 + 4u * prm.capA_s;
     const size_t spill_per_cta = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);
-    uint32_t* const Ag0 = prm.spill + (size_t)blockIdx.x * spill_per_cta + (size_t)2 * (prm.capQ - prm.capQ_s);
-    uint32_t* const Ag1 = Ag0 + (prm.capA - prm.capA_s);
+    // the host checks that the spill area has fewer than 2^32 words
+    const uint32_t qg_off = (uint32_t)((size_t)blockIdx.x * spill_per_cta);
+    const uint32_t ag_off0 = qg_off + 2u * (prm.capQ - prm.capQ_s), ag_off1 = ag_off0 + (prm.capA - prm.capA_s);
 
     __shared__ unsigned int s_sim, s_cntA[2], s_cntQ[2], s_over;
     __shared__ unsigned long long s_trials;
@@ -399,7 +401,7 @@ fire_propagate_kernel(const prop_params prm)
     step_ctx c;
     c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles; c.thr4 = reinterpret_cast<const uint4*>(prm.thr);
     c.qs_addr = qs_addr; c.capQ_s = prm.capQ_s; c.capA_s = prm.capA_s; c.capA = prm.capA;
-    c.Qg = reinterpret_cast<uint2*>(prm.spill + (size_t)blockIdx.x * spill_per_cta);
+    c.spill = prm.spill; c.qg_off = qg_off;
     c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
     const uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]), cntQ_addr = (uint32_t)__cvta_generic_to_shared(&s_cntQ[0]);
     c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
@@ -433,7 +435,7 @@ fire_propagate_kernel(const prop_params prm)
             s_over = 0u; s_trials = 0ull;
             if (valid) {
                 const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
-                if (prm.capA_s > 0) sts32(as_addr0, e0); else Ag0[0] = e0;
+                if (prm.capA_s > 0) sts32(as_addr0, e0); else prm.spill[ag_off0] = e0;
                 atomicAnd(reinterpret_cast<uint32_t*>(prm.tiles) + (((size_t)c.plane_w + (size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
         }
@@ -445,7 +447,7 @@ fire_propagate_kernel(const prop_params prm)
         while (c.nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
             const uint32_t par = t & 1u;
             c.ac_addr = par ? as_addr1 : as_addr0; c.an_addr = par ? as_addr0 : as_addr1;
-            c.Ac_g = par ? Ag1 : Ag0; c.An_g = par ? Ag0 : Ag1;
+            c.ac_off = par ? ag_off1 : ag_off0; c.an_off = par ? ag_off0 : ag_off1;
             c.cntQ = cntQ_addr + 4u * par; c.cntA_next = cntA_addr + 4u * (par ^ 1u);
 
             // ---- phase 1: susceptible neighbours of the burning cells and their thresholds -> trial queue.
@@ -589,15 +591,16 @@ fire_propagate_async_kernel(const prop_params prm)
     asm volatile("" : "+r"(ring_addr));
     const uint32_t as_addr0 = (uint32_t)__cvta_generic_to_shared(smem) + nwarps * (kRingEntries * 8u), as_addr1 = as_addr0 + 4u * prm.capA_s;
     const size_t spill_per_cta = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);
-    uint32_t* const Ag0 = prm.spill + (size_t)blockIdx.x * spill_per_cta + (size_t)2 * (prm.capQ - prm.capQ_s);
-    uint32_t* const Ag1 = Ag0 + (prm.capA - prm.capA_s);
+    // the host checks that the spill area has fewer than 2^32 words
+    const uint32_t qg_off = (uint32_t)((size_t)blockIdx.x * spill_per_cta);
+    const uint32_t ag_off0 = qg_off + 2u * (prm.capQ - prm.capQ_s), ag_off1 = ag_off0 + (prm.capA - prm.capA_s);
 
     __shared__ unsigned int s_sim, s_cntA[3], s_over;
     __shared__ unsigned long long s_trials;
 
     step_ctx c;
     c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles; c.thr4 = reinterpret_cast<const uint4*>(prm.thr);
-    c.capA_s = prm.capA_s; c.capA = prm.capA; c.capQ_s = 0u; c.qs_addr = 0u; c.Qg = nullptr; c.cntQ = 0u; c.nQ = 0u;
+    c.capA_s = prm.capA_s; c.capA = prm.capA; c.capQ_s = 0u; c.qs_addr = 0u; c.spill = prm.spill; c.qg_off = qg_off; c.cntQ = 0u; c.nQ = 0u;
     c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
     const uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]);
     c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
@@ -628,7 +631,7 @@ fire_propagate_async_kernel(const prop_params prm)
             s_cntA[0] = valid ? 1u : 0u; s_cntA[1] = 0u; s_cntA[2] = 0u; s_over = 0u; s_trials = 0ull;
             if (valid) {
                 const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
-                if (prm.capA_s > 0) sts32(as_addr0, e0); else Ag0[0] = e0;
+                if (prm.capA_s > 0) sts32(as_addr0, e0); else prm.spill[ag_off0] = e0;
                 // the ignition is burnt at t = 0: cleared in plane 0 (read by step 0); plane 1 is caught up by step 0 itself
                 atomicAnd(reinterpret_cast<uint32_t*>(plane0) + (((size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
@@ -641,7 +644,7 @@ fire_propagate_async_kernel(const prop_params prm)
         while (c.nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
             const uint32_t par = t & 1u;
             c.ac_addr = par ? as_addr1 : as_addr0; c.an_addr = par ? as_addr0 : as_addr1;
-            c.Ac_g = par ? Ag1 : Ag0; c.An_g = par ? Ag0 : Ag1;
+            c.ac_off = par ? ag_off1 : ag_off0; c.an_off = par ? ag_off0 : ag_off1;
             c.cntA_next = cntA_addr + 4u * ((t + 1u) % 3u);
             if (tid == 0) s_cntA[(t + 2u) % 3u] = 0u;             // read last at the start of step t - 1, appended to in step t + 1
             c.plane_r = plane0_t + par * (uint32_t)nt;                                        // read plane
@@ -661,7 +664,7 @@ fire_propagate_async_kernel(const prop_params prm)
                 uint32_t i = u * 32u + c.lane;
                 const bool live = i < c.nA;
                 i = live ? i : c.nA - 1u;
-                const uint32_t e = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.Ac_g + (i - c.capA_s));
+                const uint32_t e = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.spill + (c.ac_off + (i - c.capA_s)));
                 const uint32_t x = e & 0xFFFFu, y = e >> 16;
                 const uint32_t tx0 = x >> 3, ty0 = y >> 3, bx = x & 7u, by = y & 7u;
                 const uint32_t tidx = ty0 * c.Tw + tx0;
@@ -1051,6 +1054,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     // ---- scratch owned by the handle (grow-only; growing waits for the stream first)
     const size_t spill_per_cta = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);
     const size_t spill_bytes = spill_per_cta * (size_t)grid * 4 + 16;
+    if (spill_per_cta * (size_t)grid >= ((size_t)1 << 32)) return FIRE_EINVAL;   // spill slots are addressed by 32-bit word offsets
     const size_t nw = (size_t)L->H * L->Ww;
     const size_t nt = (size_t)L->Tw * L->Th;
     const size_t rescue_bytes = nw * 4 * 2 * kRescueCtas;
