@@ -348,3 +348,43 @@ def test_genetic_algorithm_drives_the_batch_api(request):
     _, fits = search.monte_carlo(ev, lo, hi, n_samples=256, batch=128, seed=12)
     assert np.isfinite(fits[0]) and fits[0] < 1.0                       # App. C: brute force finds something better than "nothing burns"
     L.close()
+
+
+# ---------------------------------------------------------------------------------- randomised parity
+def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
+    """Seeded fuzz: random lattice sizes (1 x 1 .. 140 x 200, ragged), vegetation, parameters, ignitions (some off the lattice
+    or on non-burnable cells), step limits, CTA sizes, residencies, list capacities, launch orders and both kernel families.
+    The oracle is fed the GPU's own threshold tables, so burned maps, steps and trial counts must be bit-exact."""
+    rng = np.random.default_rng(20260604)
+    n = 0
+    for it in range(60):
+        H, W = int(rng.integers(1, 140)), int(rng.integers(1, 200))
+        ls = {"veg": rng.choice(4, (H, W), p=[.15, .3, .3, .25]).astype(np.uint8),
+              "slope": (rng.random((H, W)) * 0.6).astype(np.float32),
+              "aspect": (rng.random((H, W)) * 2 * np.pi).astype(np.float32),
+              "wind": (rng.random((H, W)) * 2 * np.pi).astype(np.float32)}
+        P, S = int(rng.integers(1, 5)), int(rng.integers(1, 40))
+        betas = np.stack([[rng.uniform(-2, 1.5), rng.uniform(-1, 0), rng.uniform(-.5, .5), rng.uniform(0, 2), rng.uniform(0, 1.5)]
+                          for _ in range(P)]).astype(np.float32)
+        ign = np.stack([rng.integers(-1, W + 1, S), rng.integers(-1, H + 1, S)], 1).astype(np.int32)
+        par = rng.integers(0, P, S).astype(np.int32)
+        seeds = rng.integers(0, 2 ** 63, S).astype(np.uint64)
+        max_steps = int(rng.choice([0, 0, 0, 3, 17]))
+        geom = (int(rng.choice([32, 64, 96, 128, 256, 512, 1024])), int(rng.integers(1, 9)))
+        caps = (int(rng.choice([0, 0, 1, 4, 16])), int(rng.choice([0, 0, 0, 2, 64])))
+        mode = int(rng.choice([0, 1, 128, 129, 144, 145]))
+        Lo = orc_landscape(orc, ls)
+        L = gh.make_landscape(ls)
+        gh.upload(L, betas)
+        tables = [gh.thresholds(L, p) for p in range(P)]
+        o = orc.simulate_batch(Lo, betas, ign, par, seeds, max_steps=max_steps, tables=tables)
+        lf.fire_set_launch_geometry(L, *geom)
+        lf.fire_set_list_capacity(L, *caps)
+        lf.fire_set_schedule(L, mode)
+        g = gh.simulate(L, ign, par, seeds, max_steps=max_steps)
+        what = (it, H, W, P, S, max_steps, geom, caps, mode)
+        assert (g["burned"] == o["burned"]).all(), what
+        assert (g["steps"] == o["steps"]).all() and (g["trials"] == o["trials"]).all(), what
+        n += 1
+        L.close()
+    report(request, cases=n)
