@@ -45,7 +45,7 @@ METRIC = "cell-neighbour trials/s"
 UNIT = "trials/s"
 # ncu --set full capture of fire_propagate_kernel on the workload below, dram__bytes_read.sum + dram__bytes_write.sum
 # per launch (profiles/README.md names the file and the command).  None until a capture exists for that config.
-NCU_TRAFFIC_BYTES = {3: 17595626000 + 208820224}      # profiles/r1_v2c_propagate_ncu.md, final build
+NCU_TRAFFIC_BYTES = {3: 17498318000 + 201962752}      # profiles/r1_v2c_propagate_ncu.md, final build
 
 
 def log(*a):
