@@ -599,14 +599,16 @@ fire_propagate_async_kernel(const prop_params prm)
     const uint32_t qg_off = (uint32_t)((size_t)blockIdx.x * spill_per_cta);
     const uint32_t ag_off0 = qg_off + 2u * (prm.capQ - prm.capQ_s), ag_off1 = ag_off0 + (prm.capA - prm.capA_s);
 
-    __shared__ unsigned int s_sim, s_cntA[3], s_over;
+    __shared__ struct { unsigned int cntA[3], over, sim; } s_ctl;        // counters in one block: one base address
+    unsigned int (&s_cntA)[3] = s_ctl.cntA; unsigned int& s_over = s_ctl.over; unsigned int& s_sim = s_ctl.sim;
     __shared__ unsigned long long s_trials;
 
     step_ctx c;
     c.W = (uint32_t)prm.W; c.Tw = (uint32_t)prm.Tw; c.Th = (uint32_t)prm.Th; c.tiles = prm.tiles; c.thr4 = reinterpret_cast<const uint4*>(prm.thr);
     c.capA_s = prm.capA_s; c.capA = prm.capA; c.capQ_s = 0u; c.qs_addr = 0u; c.spill = prm.spill; c.qg_off = qg_off; c.cntQ = 0u; c.nQ = 0u;
-    c.over = (uint32_t)__cvta_generic_to_shared(&s_over);
-    const uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]);
+    uint32_t cntA_addr = (uint32_t)__cvta_generic_to_shared(&s_cntA[0]);
+    asm volatile("" : "+r"(cntA_addr));          // as for ring_addr
+    c.over = cntA_addr + 12u;
     c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
     const size_t nt = (size_t)c.Tw * c.Th;
 
