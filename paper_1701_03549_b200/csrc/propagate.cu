@@ -133,6 +133,7 @@ struct step_ctx {
     const uint64_t* tiles;
     uint32_t plane_r;             // tile offset of the plane this step READS
     uint32_t plane_w;             // tile offset of the plane this step UPDATES (the same plane in the two-phase kernel)
+    uint32_t plane_w2;            // the same in 8 x 4-cell half tiles (2 * plane_w), kept in a register for the atomics
     const uint4* thr4;            // the threshold table (kernel parameter), 2 x uint4 per sector
     uint32_t thr_sec;             // first sector of this simulation's parameter vector (a table that fits in HBM has < 2^32 sectors)
     // lists
@@ -306,7 +307,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
         const uint32_t rnd = (d & 2u) ? hi : lo;
         pt.old[u] = 0u;
         if (fire_trial(rnd, T[u])) {
-            pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + ((c.plane_w << 1) + widx), ~(1u << pt.bit[u]));
+            pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + (c.plane_w2 + widx), ~(1u << pt.bit[u]));
 #ifdef FIRE_PREFETCH_THR
             asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)(c.thr_sec + cell) * 2));
 #endif
@@ -425,6 +426,8 @@ fire_propagate_kernel(const prop_params prm)
         const uint64_t seed = prm.seeds[s];
         const uint32_t sim = prm.sim_ids ? (uint32_t)prm.sim_ids[s] : s;
         c.plane_r = c.plane_w = s * (c.Tw * c.Th);             // the host checks that S * tiles fits 31 bits
+        c.plane_w2 = c.plane_w << 1;
+        asm volatile("" : "+r"(c.plane_w2));                  // once per simulation, used once per unit of trials
         bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
         if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
         c.thr_sec = valid ? (uint32_t)p * (c.W * (uint32_t)prm.H) : 0u;
@@ -567,7 +570,7 @@ __device__ __forceinline__ void trials_issue_ring(const step_ctx& c, const philo
         }
         const uint32_t lo = (d & 1u) ? c1 : c0, hi = (d & 1u) ? c3 : c2;
         const uint32_t rnd = (d & 2u) ? hi : lo;
-        if (fire_trial(rnd, T[u])) pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + ((c.plane_w << 1) + widx), ~(1u << pt.bit[u]));
+        if (fire_trial(rnd, T[u])) pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + (c.plane_w2 + widx), ~(1u << pt.bit[u]));
     }
 }
 
@@ -655,6 +658,7 @@ fire_propagate_async_kernel(const prop_params prm)
             if (tid == 0) s_cntA[(t + 2u) % 3u] = 0u;             // read last at the start of step t - 1, appended to in step t + 1
             c.plane_r = plane0_t + par * (uint32_t)nt;                                        // read plane
             c.plane_w = plane0_t + (par ^ 1u) * (uint32_t)nt;                                 // written plane
+            c.plane_w2 = c.plane_w << 1;
 
             philox_step ph;
 #pragma unroll
