@@ -134,10 +134,13 @@ int fire_set_list_capacity(fire_landscape* L, int32_t shared_entries, int32_t to
 
 /* Tuning knob / test hook (pin P-9): order in which the simulations of a batch are handed to the resident
  * CTAs.  0 = default: largest expected fires first (by the mean contagion probability of their parameter
- * vector, a by-product of fire_params_upload); 1 = batch order.  Bits 4.. (mode >> 4) pick the propagation kernel:
- * 0 = automatic, 8 = asynchronous-warp kernel (two state planes, one barrier per step), 9 = two-phase kernel (one
- * state plane, shared trial queue), 1..2 = other instantiations of the two-phase kernel.  Results never depend on it. */
+ * vector, a by-product of fire_params_upload); 1 = batch order.  Results never depend on it. */
 int fire_set_schedule(fire_landscape* L, int32_t mode);
+
+/* Test hook (pin P-9): which propagation kernel fire_simulate_batch launches.  0 = automatic (by batch size),
+ * 1 = two-phase kernel (one CTA per simulation, one state plane, two block barriers per step), 2 = asynchronous-warp
+ * kernel (one CTA per simulation, two state planes, one block barrier per step).  Results never depend on it. */
+int fire_set_kernel(fire_landscape* L, int32_t family);
 
 const char* fire_error_string(int code);
 

@@ -62,7 +62,7 @@ struct fire_landscape {
     int threads_per_cta;          // 0 = default
     int ctas_per_sm;              // 0 = default
     int list_capacity;            // total frontier-list capacity per CTA (0 = default); tests shrink it to force the rescue path
-    int kernel_variant;           // tuning: which instantiation of the propagation kernel (0 = default)
+    int kernel_family;            // fire_set_kernel: 0 = automatic, 1 = two-phase kernel, 2 = asynchronous-warp kernel
     int schedule;                 // 0 = largest expected fires first, 1 = batch order
     int list_shared;              // shared-memory part of it (0 = default); tests shrink it to force the global spill
 

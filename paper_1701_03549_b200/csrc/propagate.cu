@@ -787,42 +787,46 @@ fire_burnable_tiles_kernel(const uint32_t* __restrict__ burnable, int H, int Ww,
 }
 
 __global__ void __launch_bounds__(256)
-fire_init_tiles_kernel(const uint64_t* __restrict__ burnable_tiles, uint64_t* __restrict__ tiles, size_t nt)
+fire_init_tiles_kernel(const uint64_t* __restrict__ burnable_tiles, uint64_t* __restrict__ tiles, size_t nt, size_t nplanes)
 {
-    uint64_t* const plane = tiles + (size_t)blockIdx.y * nt;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
-    if ((nt & 1) == 0) {
-        const uint4* const b4 = reinterpret_cast<const uint4*>(burnable_tiles);
-        uint4* const p4 = reinterpret_cast<uint4*>(plane);
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nt / 2; i += stride) p4[i] = __ldg(b4 + i);
-    } else {
-        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += stride) plane[i] = __ldg(burnable_tiles + i);
+    for (size_t pl = blockIdx.y; pl < nplanes; pl += gridDim.y) {      // gridDim.y <= 65535 whatever the batch size
+        uint64_t* const plane = tiles + pl * nt;
+        if ((nt & 1) == 0) {
+            const uint4* const b4 = reinterpret_cast<const uint4*>(burnable_tiles);
+            uint4* const p4 = reinterpret_cast<uint4*>(plane);
+            for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nt / 2; i += stride) p4[i] = __ldg(b4 + i);
+        } else {
+            for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += stride) plane[i] = __ldg(burnable_tiles + i);
+        }
     }
 }
 
 // one thread per (tile row, bitmap word column): 4 tiles in (32 B), 8 words out (one per lattice row)
 __global__ void __launch_bounds__(256)
 fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __restrict__ tiles, const uint32_t* __restrict__ plane_sel,
-                   int planes, uint32_t* __restrict__ out_burned, int H, int Ww, int Tw, int Th)
+                   int planes, uint32_t* __restrict__ out_burned, int H, int Ww, int Tw, int Th, int S)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= Th * Ww) return;
     const int ty = i / Ww, wx = i % Ww;
-    const size_t plane = (size_t)blockIdx.y * planes + (planes > 1 ? (plane_sel[blockIdx.y] & 1u) : 0u);
-    const uint64_t* const row = tiles + plane * Tw * Th + (size_t)ty * Tw;
-    uint64_t tl[4];
+    for (int s = blockIdx.y; s < S; s += gridDim.y) {                  // gridDim.y <= 65535 whatever the batch size
+        const size_t plane = (size_t)s * planes + (planes > 1 ? (plane_sel[s] & 1u) : 0u);
+        const uint64_t* const row = tiles + plane * Tw * Th + (size_t)ty * Tw;
+        uint64_t tl[4];
 #pragma unroll
-    for (int k = 0; k < 4; ++k) tl[k] = (4 * wx + k < Tw) ? __ldcs(reinterpret_cast<const unsigned long long*>(row + 4 * wx + k)) : 0ull;
-    uint32_t* const out = out_burned + (size_t)blockIdx.y * H * Ww;
+        for (int k = 0; k < 4; ++k) tl[k] = (4 * wx + k < Tw) ? __ldcs(reinterpret_cast<const unsigned long long*>(row + 4 * wx + k)) : 0ull;
+        uint32_t* const out = out_burned + (size_t)s * H * Ww;
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-        const int y = ty * 8 + r;
-        if (y < H) {
-            uint32_t susw = 0u;
+        for (int r = 0; r < 8; ++r) {
+            const int y = ty * 8 + r;
+            if (y < H) {
+                uint32_t susw = 0u;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) susw |= (uint32_t)((tl[k] >> (8 * r)) & 0xFFull) << (8 * k);
-            const size_t wi = (size_t)y * Ww + wx;
-            out[wi] = __ldg(burnable + wi) & ~susw;
+                for (int k = 0; k < 4; ++k) susw |= (uint32_t)((tl[k] >> (8 * r)) & 0xFFull) << (8 * k);
+                const size_t wi = (size_t)y * Ww + wx;
+                out[wi] = __ldg(burnable + wi) & ~susw;
+            }
         }
     }
 }
@@ -999,7 +1003,13 @@ extern "C" int fire_set_schedule(fire_landscape* L, int32_t mode)
 {
     if (L == nullptr || mode < 0) return FIRE_EINVAL;
     L->schedule = mode & 1;
-    L->kernel_variant = mode >> 4;       // tuning builds: bits 4.. select an instantiation of the kernel
+    return FIRE_OK;
+}
+
+extern "C" int fire_set_kernel(fire_landscape* L, int32_t family)
+{
+    if (L == nullptr || family < 0 || family > 2) return FIRE_EINVAL;
+    L->kernel_family = family;
     return FIRE_OK;
 }
 
@@ -1029,47 +1039,46 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         if (per_sm == 0) per_sm = (1024 / threads) > 0 ? (1024 / threads) : 1;
     }
     const int grid = (int)((long long)S < (long long)L->num_sms * per_sm ? S : L->num_sms * per_sm);
+    // kernel family (fire_set_kernel): 1 = two-phase kernel (one state plane, two block barriers per step), 2 = asynchronous-warp
+    // kernel (two state planes, one barrier per step, per-warp trial rings); 0 = the two-phase kernel for batches that fill the GPU
+    // with 256-thread CTAs, the asynchronous-warp kernel for small batches of large fires (wide CTAs, long fronts)
+    const bool async = L->kernel_family == 2 || (L->kernel_family == 0 && threads >= 512 && L->threads_per_cta == 0);
+    const int planes = async ? 2 : 1;
     prop_params prm;
+    uint32_t capA = L->list_capacity ? (uint32_t)L->list_capacity : 0u;
+    if (capA == 0) {
+        // generous: the burning front of a W x H lattice is a curve, not an area
+        size_t want = (size_t)8 * (size_t)(L->W + L->H);
+        if (want < 8192) want = 8192;
+        if (want > L->cells) want = L->cells;
+        capA = (uint32_t)want;
+    }
+    if (capA < 1) capA = 1;
     uint32_t capA_s = 1536u;                                   // 24 B of shared memory per entry (two lists + 2 queue slots)
     {
         const uint32_t fit = (uint32_t)((180u * 1024u) / ((uint32_t)per_sm * 24u)) & ~127u;
         if (capA_s > fit) capA_s = fit < 128u ? 128u : fit;
     }
     if (L->list_shared) capA_s = (uint32_t)L->list_shared;
-    uint32_t capA = L->list_capacity ? (uint32_t)L->list_capacity : 0u;
-    if (capA == 0) {
-        // generous: a BFS level set of an open W x H lattice has at most 2(W+H) cells
-        size_t want = (size_t)16 * (size_t)(L->W + L->H);
-        if (want < 8192) want = 8192;
-        if (want > L->cells) want = L->cells;
-        capA = (uint32_t)want;
-    }
-    if (capA < 1) capA = 1;
     if (capA_s > capA) capA_s = capA;
     prm.capA_s = capA_s; prm.capA = capA;
     prm.capQ = 8u * capA;
     prm.capQ_s = 2u * capA_s;                                  // default: 1536-cell lists + 3072-trial queue = 36 KiB per CTA
-    if (prm.capQ_s > prm.capQ) prm.capQ_s = prm.capQ;
-    // kernel family: 0 = two-phase kernel (one state plane, two barriers per step); 1 = asynchronous-warp kernel
-    // (two state planes, one barrier per step, per-warp trial rings)
-    // Default: the two-phase kernel for batches that fill the GPU with 256-thread CTAs; the asynchronous-warp kernel for
-    // small batches of large fires (wide CTAs), whose trial queues would not fit in shared memory.  fire_set_schedule
-    // bits 4.. force one: 8 = asynchronous-warp, 9 = two-phase.
-    const bool async = L->kernel_variant == 8 || (L->kernel_variant != 9 && L->kernel_variant < 8 && threads >= 512 && L->threads_per_cta == 0);
-    const int planes = async ? 2 : 1;
     const size_t smem = async ? ((size_t)(threads / 32) * kRingEntries * 8 + (size_t)2 * prm.capA_s * sizeof(uint32_t))
                               : ((size_t)2 * prm.capA_s + (size_t)2 * prm.capQ_s) * sizeof(uint32_t);
-    if (smem > 200 * 1024) return FIRE_EINVAL;
+    if (prm.capQ_s > prm.capQ) prm.capQ_s = prm.capQ;
+    if (smem > (size_t)227 * 1024 - 1024) return FIRE_EINVAL;
 
-    // ---- scratch owned by the handle (grow-only; growing waits for the stream first)
-    const size_t spill_per_cta = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);
-    const size_t spill_bytes = spill_per_cta * (size_t)grid * 4 + 16;
-    if (spill_per_cta * (size_t)grid >= ((size_t)1 << 32)) return FIRE_EINVAL;   // spill slots are addressed by 32-bit word offsets
+    // ---- scratch owned by the handle (grow-only; growing waits for the stream first: see fire.h)
+    const size_t spill_per_list_set = (size_t)2 * (prm.capQ - prm.capQ_s) + (size_t)2 * (prm.capA - prm.capA_s);   // per CTA
+    const size_t spill_sets = (size_t)grid;
+    const size_t spill_bytes = spill_per_list_set * spill_sets * 4 + 16;
+    if (spill_per_list_set * spill_sets >= ((size_t)1 << 32)) return FIRE_EINVAL;   // spill slots are addressed by 32-bit word offsets
     const size_t nw = (size_t)L->H * L->Ww;
     const size_t nt = (size_t)L->Tw * L->Th;
     const size_t rescue_bytes = nw * 4 * 2 * kRescueCtas;
-    if (nt * (size_t)S * 2 >= ((size_t)1 << 31)) return FIRE_EINVAL;   // planes are addressed by 32-bit tile offsets: split the batch
-    const size_t tiles_bytes = nt * 8 * (size_t)S * 2;        // room for two planes per simulation
+    if (nt * (size_t)S * planes >= ((size_t)1 << 31)) return FIRE_EINVAL;   // planes are addressed by 32-bit tile offsets: split the batch
+    const size_t tiles_bytes = nt * 8 * (size_t)S * planes;
     if (L->status_capacity < (size_t)2 * S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes ||
         L->tiles_capacity < tiles_bytes || L->order_capacity < (size_t)S * 4 || L->burnable_tiles == nullptr) {
         FIRE_CUDA_TRY(L, cudaStreamSynchronize(st));
@@ -1106,7 +1115,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.Tw = L->Tw; prm.Th = L->Th; prm.num_sms = L->num_sms;
     prm.max_steps = max_steps;
 
-    // ---- launch order: largest expected fires first (only matters when there are more simulations than resident CTAs)
+    // ---- launch order: largest expected fires first (only matters when there are more simulations than resident ones)
     prm.order = nullptr;
     if (S > grid && L->param_mean != nullptr && L->schedule == 0) {
         fire_order_kernel<<<1, 1024, 0, st>>>(sim_param, L->param_mean, S, L->P, 1.0f / ((float)L->cells * 8.0f), L->order);
@@ -1121,37 +1130,20 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         unsigned chunks = (unsigned)((units + 256 * 4 - 1) / (256 * 4));
         if (chunks < 1) chunks = 1;
         if (chunks > 64) chunks = 64;
-        fire_init_tiles_kernel<<<dim3(chunks, (unsigned)(S * planes)), 256, 0, st>>>(L->burnable_tiles, L->tiles, nt);
+        const size_t nplanes = (size_t)S * planes;
+        fire_init_tiles_kernel<<<dim3(chunks, (unsigned)(nplanes < 65535 ? nplanes : 65535)), 256, 0, st>>>(L->burnable_tiles, L->tiles, nt, nplanes);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
     FIRE_CUDA_TRY(L, cudaMemsetAsync(L->work_counter, 0, 4 * sizeof(unsigned int), st));
     if (async) FIRE_CUDA_TRY(L, cudaMemsetAsync(L->status + S, 0, (size_t)S * 4, st));
-    void (*kernel)(const prop_params) = fire_propagate_kernel<1024, 1, 2, 4>;
-    const int variant = L->kernel_variant;
-    if (threads <= 256 && per_sm >= 8)
-        kernel = variant == 1 ? fire_propagate_kernel<256, 8, 1, 1> : (variant == 2 ? fire_propagate_kernel<256, 8, 1, 4> : fire_propagate_kernel<256, 8, 1, 2>);
-    else if (threads <= 256 && per_sm >= 6)
-        kernel = variant == 1 ? fire_propagate_kernel<256, 6, 1, 2> : (variant == 2 ? fire_propagate_kernel<256, 6, 1, 4> : fire_propagate_kernel<256, 6, 2, 4>);
-    else if (threads <= 256 && per_sm == 5)
-        kernel = variant == 1 ? fire_propagate_kernel<256, 5, 1, 2> : (variant == 2 ? fire_propagate_kernel<256, 5, 1, 4> : fire_propagate_kernel<256, 5, 2, 4>);
-    else if (threads <= 256 && per_sm == 3) kernel = fire_propagate_kernel<256, 3, 2, 4>;
-    else if (threads <= 256)
-        kernel = variant == 2 ? fire_propagate_kernel<256, 4, 1, 4> : fire_propagate_kernel<256, 4, 2, 4>;
-    else if (threads <= 512 && per_sm >= 4) kernel = variant == 1 ? fire_propagate_kernel<512, 4, 1, 1> : fire_propagate_kernel<512, 4, 1, 2>;
-    else if (threads <= 512 && per_sm == 3) kernel = fire_propagate_kernel<512, 3, 1, 4>;
-    else if (threads <= 512) kernel = fire_propagate_kernel<512, 2, 2, 4>;
-    else if (per_sm >= 2) kernel = fire_propagate_kernel<1024, 2, 1, 2>;
-    if (async) {
-        if (threads <= 256 && per_sm >= 6) kernel = fire_propagate_async_kernel<256, 6>;
-        else if (threads <= 256 && per_sm == 5) kernel = fire_propagate_async_kernel<256, 5>;
-        else if (threads <= 256) kernel = fire_propagate_async_kernel<256, 4>;
-        else if (threads <= 512) kernel = fire_propagate_async_kernel<512, 2>;
-        else kernel = fire_propagate_async_kernel<1024, 1>;
-    }
+    // instantiations differ in their register budget only (threads <= kMaxThreads is the one hard constraint)
+    void (*kernel)(const prop_params) = nullptr;
+    if (async) kernel = threads <= 256 ? fire_propagate_async_kernel<256, 4> : (threads <= 512 ? fire_propagate_async_kernel<512, 2> : fire_propagate_async_kernel<1024, 1>);
+    else kernel = threads <= 256 ? (per_sm <= 4 ? fire_propagate_kernel<256, 4, 2, 4> : fire_propagate_kernel<256, 8, 1, 2>)
+                                 : (threads <= 512 ? fire_propagate_kernel<512, 2, 2, 4> : fire_propagate_kernel<1024, 1, 2, 4>);
     if (smem + 1024 > 48 * 1024)                     // dynamic + static shared memory beyond the default limit
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    {   // ask for just the shared memory the resident CTAs need, so that the rest of the 228 KB stays L1 (the in-flight
-        // sector and tile loads of phase 1 live there)
+    {   // ask for just the shared memory the resident CTAs need, so that the rest of the 228 KB stays L1
         int pct = (int)(((size_t)per_sm * (smem + 1024 + 256) * 100 + 228 * 1024 - 1) / (228 * 1024));   // + 1 KiB reserved per CTA + static shared memory
         if (pct > 100) pct = 100;
         FIRE_CUDA_TRY(L, cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct));
@@ -1163,8 +1155,8 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     if (prof) { FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count + 1], st)); L->prof_count += 1; }
     {
         const size_t n = (size_t)L->Th * L->Ww;
-        fire_finish_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)S), 256, 0, st>>>(L->burnable, L->tiles, L->status + S, planes, out_burned,
-                                                                                          L->H, L->Ww, L->Tw, L->Th);
+        fire_finish_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)(S < 65535 ? S : 65535)), 256, 0, st>>>(L->burnable, L->tiles, L->status + S, planes, out_burned,
+                                                                                          L->H, L->Ww, L->Tw, L->Th, S);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
     fire_propagate_rescue_kernel<<<kRescueCtas, 256, 0, st>>>(prm, L->rescue_planes);

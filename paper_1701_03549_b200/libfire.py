@@ -21,7 +21,7 @@ FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
     "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
-    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_error_string",
+    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
 
@@ -59,6 +59,7 @@ def load() -> C.CDLL:
     lib.fire_set_launch_geometry.argtypes = [_vp, C.c_int32, C.c_int32]
     lib.fire_set_list_capacity.argtypes = [_vp, C.c_int32, C.c_int32]
     lib.fire_set_schedule.argtypes = [_vp, C.c_int32]
+    lib.fire_set_kernel.argtypes = [_vp, C.c_int32]
     lib.fire_set_profiling.argtypes = [_vp, C.c_int32]
     lib.fire_profile_read.argtypes = [_vp, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
     lib.fire_error_string.argtypes = [C.c_int]
@@ -234,6 +235,10 @@ def fire_set_launch_geometry(L: Landscape, threads_per_cta: int = 0, ctas_per_sm
 
 def fire_set_schedule(L: Landscape, mode: int = 0) -> None:
     _check(load().fire_set_schedule(L.handle, int(mode)), "fire_set_schedule")
+
+
+def fire_set_kernel(L: Landscape, family: int = 0) -> None:
+    _check(load().fire_set_kernel(L.handle, int(family)), "fire_set_kernel")
 
 
 def fire_set_list_capacity(L: Landscape, shared_entries: int = 0, total_entries: int = 0) -> None:

@@ -217,20 +217,24 @@ def test_results_do_not_depend_on_launch_geometry_or_list_capacity(request):
     base = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
     again = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
     assert (base["burned"] == again["burned"]).all()
-    # mode: bit 0 = batch order instead of largest-expected-first; 128 / 144 force the asynchronous-warp / two-phase kernel
-    for threads, per_sm, shared, total, mode in [(32, 1, 0, 0, 0), (64, 8, 0, 0, 1), (128, 2, 0, 0, 0), (512, 1, 0, 0, 144), (1024, 1, 0, 0, 145),
-                                                 (256, 4, 16, 0, 0), (256, 4, 5, 4096, 1), (96, 3, 1, 0, 0), (256, 4, 8, 8, 0),
-                                                 (128, 4, 64, 100, 1), (256, 2, 0, 1, 0), (256, 5, 0, 0, 0), (256, 6, 0, 0, 1),
-                                                 (256, 8, 768, 0, 0), (128, 1, 0, 0, 1),
-                                                 (256, 4, 0, 0, 128), (32, 2, 0, 0, 129), (1024, 1, 0, 0, 128), (512, 2, 16, 0, 128),
-                                                 (256, 5, 5, 4096, 129), (256, 6, 8, 8, 128), (128, 4, 1, 1, 128), (0, 0, 0, 0, 128)]:
+    # (threads per CTA, CTAs per SM, shared list entries, total list entries, launch order, kernel family)
+    # family 0 = automatic, 1 = two-phase kernel, 2 = asynchronous-warp kernel
+    for threads, per_sm, shared, total, order, family in [
+            (32, 1, 0, 0, 0, 0), (64, 8, 0, 0, 1, 0), (128, 2, 0, 0, 0, 0), (512, 1, 0, 0, 0, 1), (1024, 1, 0, 0, 1, 1),
+            (256, 4, 16, 0, 0, 0), (256, 4, 5, 4096, 1, 0), (96, 3, 1, 0, 0, 0), (256, 4, 8, 8, 0, 0),
+            (128, 4, 64, 100, 1, 0), (256, 2, 0, 1, 0, 0), (256, 5, 0, 0, 0, 0), (256, 6, 0, 0, 1, 0),
+            (256, 8, 768, 0, 0, 0), (128, 1, 0, 0, 1, 0), (128, 16, 0, 0, 0, 1), (0, 0, 0, 0, 0, 1),
+            (256, 4, 0, 0, 0, 2), (32, 2, 0, 0, 1, 2), (1024, 1, 0, 0, 0, 2), (512, 2, 16, 0, 0, 2),
+            (256, 5, 5, 4096, 1, 2), (256, 6, 8, 8, 0, 2), (128, 4, 1, 1, 0, 2), (0, 0, 0, 0, 0, 2)]:
+        mode = (threads, per_sm, shared, total, order, family)
         lf.fire_set_launch_geometry(L, threads, per_sm)
         lf.fire_set_list_capacity(L, shared, total)
-        lf.fire_set_schedule(L, mode)
+        lf.fire_set_schedule(L, order)
+        lf.fire_set_kernel(L, family)
         g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
         ok = (g["burned"] == base["burned"]).all(axis=(1, 2))
-        assert ok.all(), f"geometry {(threads, per_sm, shared, total, mode)}: sims {np.flatnonzero(~ok)[:10]} differ"
-        assert (g["steps"] == base["steps"]).all() and (g["trials"] == base["trials"]).all(), (threads, per_sm, shared, total, mode)
+        assert ok.all(), f"geometry {mode}: sims {np.flatnonzero(~ok)[:10]} differ"
+        assert (g["steps"] == base["steps"]).all() and (g["trials"] == base["trials"]).all(), mode
     L.close()
 
 
@@ -372,7 +376,8 @@ def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
         max_steps = int(rng.choice([0, 0, 0, 3, 17]))
         geom = (int(rng.choice([32, 64, 96, 128, 256, 512, 1024])), int(rng.integers(1, 9)))
         caps = (int(rng.choice([0, 0, 1, 4, 16])), int(rng.choice([0, 0, 0, 2, 64])))
-        mode = int(rng.choice([0, 1, 128, 129, 144, 145]))
+        order, family = int(rng.integers(0, 2)), int(rng.choice([0, 1, 2]))
+        mode = (order, family)
         Lo = orc_landscape(orc, ls)
         L = gh.make_landscape(ls)
         gh.upload(L, betas)
@@ -380,7 +385,8 @@ def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
         o = orc.simulate_batch(Lo, betas, ign, par, seeds, max_steps=max_steps, tables=tables)
         lf.fire_set_launch_geometry(L, *geom)
         lf.fire_set_list_capacity(L, *caps)
-        lf.fire_set_schedule(L, mode)
+        lf.fire_set_schedule(L, order)
+        lf.fire_set_kernel(L, family)
         g = gh.simulate(L, ign, par, seeds, max_steps=max_steps)
         what = (it, H, W, P, S, max_steps, geom, caps, mode)
         assert (g["burned"] == o["burned"]).all(), what
