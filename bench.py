@@ -20,7 +20,9 @@ roofline= the propagation kernel (fire_propagate_kernel) alone: algorithmic byte
           mean launch duration, measured with CUDA events recorded by the library on the launching stream.
 N > 1   : simulations are independent -> every rank runs its own generation of S sims
           (replicates r*S .. r*S+S-1 of the same vectors: other seeds, other sim ids), no data-path collective;
-          one all-gather of the S x 4 B scores per step hands them to the GA's rank.  scaling = "weak".
+          one all-gather of the S x 4 B scores per step hands them to the GA's rank.  scaling = "weak" (default).
+          --scaling strong: ONE generation partitioned by parameter vector: rank r uploads only its P / N
+          vectors, so it builds P / N of the threshold table, and simulates their sims with batch positions as sim ids.
 
 --impl reference : this tier has no reference implementation; that arm times the CPU oracle (oracle/) as it
 stands, on a bounded sample of the same workload, on the host cores (rank 0 only).
@@ -43,9 +45,11 @@ if str(ROOT) not in sys.path:
 
 METRIC = "cell-neighbour trials/s"
 UNIT = "trials/s"
-# ncu --set full capture of fire_propagate_kernel on the workload below, dram__bytes_read.sum + dram__bytes_write.sum
-# per launch (profiles/README.md names the file and the command).  None until a capture exists for that config.
-NCU_TRAFFIC_BYTES = {3: 17498318000 + 201962752}      # profiles/r1_v2c_propagate_ncu.md, final build
+# ncu --set full capture of the propagation kernel on the workload below: dram__bytes_read.sum + dram__bytes_write.sum per
+# launch, with the commit the captured kernel was built from (profiles/README.md names the file and the command).  Refresh
+# the number together with every change of the propagation kernel; None until a capture exists for that config.
+NCU_TRAFFIC_BYTES = {3: 17482102000 + 204184320}      # profiles/r2_base_propagate_ncu.md, kernel as of commit b2a319d
+NCU_TRAFFIC_SOURCE = {3: "profiles/r2_base_propagate_ncu.md (ncu --set full, kernel of commit b2a319d)"}
 
 
 def log(*a):
@@ -54,16 +58,18 @@ def log(*a):
 
 # ------------------------------------------------------------------------------------------ oracle arm
 def oracle_sample(cfg: int, budget_sims: int):
-    """The bounded sample of the workload the CPU oracle is timed on: the first `budget_sims` simulations."""
+    """The bounded sample of the workload the CPU oracle is timed on: `budget_sims` simulations taken at a constant stride over
+    the whole batch (so every region of the parameter-vector axis is represented), with their own batch positions as sim ids."""
     from paper_1701_03549_b200 import workloads as wl
     w = wl.load_workload(cfg)
     n = min(budget_sims, w.S)
-    return w, n
+    idx = (np.arange(n, dtype=np.int64) * w.S) // n
+    return w, idx
 
 
-def time_oracle(w, n: int, repeats: int = 1):
-    """Oracle as it stands (OpenMP over sims, thresholds on demand, Eq. 2 counts per sim).  Returns
-    (trials, seconds per pass, threads)."""
+def time_oracle(w, idx, repeats: int = 1, nthreads: int = 0):
+    """Oracle as it stands (OpenMP over sims, thresholds on demand, Eq. 2 counts per sim) on the sims `idx` of the batch.
+    Returns (trials, seconds per pass, threads)."""
     from oracle import fire_oracle as orc
     orc.build()
     ls = w.landscape
@@ -73,8 +79,8 @@ def time_oracle(w, n: int, repeats: int = 1):
     trials = threads = 0
     for _ in range(repeats):
         t0 = time.perf_counter()
-        r = orc.simulate_batch(Lo, w.betas, w.ignitions[:n], w.sim_param[:n], w.seeds[:n],
-                               sim_index=np.arange(n, dtype=np.int32))
+        r = orc.simulate_batch(Lo, w.betas, w.ignitions[idx], w.sim_param[idx], w.seeds[idx],
+                               sim_index=idx.astype(np.int32), nthreads=nthreads)
         orc.fitness(ref, r["burned"], Lo.W, w.metric)
         dt = time.perf_counter() - t0
         trials, threads = int(r["trials"].sum()), int(r["threads"])
@@ -82,26 +88,34 @@ def time_oracle(w, n: int, repeats: int = 1):
     return trials, best, threads
 
 
+def sample_text(w, idx) -> str:
+    if len(idx) == w.S:
+        return f"all {w.S} simulations of {w.name} (+ Eq. 2 counts)"
+    return (f"{len(idx)} of {w.S} simulations of {w.name}, every {w.S // len(idx)}th of the batch (+ Eq. 2 counts); "
+            f"the rate is EXTRAPOLATED from this sample to the whole batch")
+
+
 def sample_budget(cfg: int) -> int:
-    # about 10-30 s of oracle work on 8 cores (measured ~15 M trials/s): cfg3 mean 0.94 M trials per sim
-    return {1: 64, 2: 256, 3: 256, 4: 4096, 5: 2}[cfg]
+    # about 10-30 s of oracle work on the GPU box's 16 host threads (measured ~73 M trials/s): cfg3 mean 0.94 M trials per sim
+    return {1: 64, 2: 256, 3: 1024, 4: 8192, 5: 4}[cfg]
 
 
 def run_reference(args) -> None:
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w, n = oracle_sample(args.cfg, sample_budget(args.cfg))
+    w, idx = oracle_sample(args.cfg, sample_budget(args.cfg))
+    n = len(idx)
     for _ in range(min(args.warmup, 1)):                 # the oracle has no caches to warm beyond page-in
-        time_oracle(w, max(1, n // 16))
+        time_oracle(w, idx[:: 16])
     per_step = []
     trials = threads = 0
     for _ in range(args.steps):
-        trials, dt, threads = time_oracle(w, n)
+        trials, dt, threads = time_oracle(w, idx)
         per_step.append(dt)
     total = float(np.sum(per_step))
     value = trials * args.steps / total
-    sample = f"first {n} of {w.S} simulations of {w.name} per step (+ Eq. 2 counts)"
+    sample = sample_text(w, idx) + " per step"
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -178,6 +192,9 @@ def run_ours(args) -> None:
         raise RuntimeError("bench.py needs a CUDA device: libfire has no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
+        # NCCL's own account of the communicator (ranks, transports, NVLS) goes to stderr: stdout carries the one JSON line
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     if rank == 0:
         fire_build.build()
@@ -208,25 +225,27 @@ def run_ours(args) -> None:
             a = a.view(np.int64)
         return torch.from_numpy(a.copy()).pin_memory()
 
-    # rank r simulates replicates r*S .. r*S+S-1 of the same population (weak scaling)
-    sim_ids_np = (np.arange(S, dtype=np.int64) + rank * S).astype(np.int32)
-    seeds_np = (np.uint64(cfg) << np.uint64(32)) | (np.arange(S, dtype=np.uint64) + np.uint64(rank * S))
-    if rank == 0:
-        assert (seeds_np == w.seeds).all()
+    strong = args.scaling == "strong"
+    if strong:
+        # ONE generation partitioned by parameter vector: rank r builds only its P / N slice of the threshold table
+        # and runs the sims of those vectors, with their batch positions as sim ids (so every fire is the full batch's fire)
+        sh = wl.shard_by_param(w, rank, world)
+        l_betas, l_ign, l_par, seeds_np, sim_ids_np, l_index = sh.betas, sh.ignitions, sh.sim_param, sh.seeds, sh.sim_ids, sh.index
+    else:
+        # rank r simulates replicates r*S .. r*S+S-1 of the same population (weak scaling)
+        sim_ids_np = (np.arange(S, dtype=np.int64) + rank * S).astype(np.int32)
+        seeds_np = (np.uint64(cfg) << np.uint64(32)) | (np.arange(S, dtype=np.uint64) + np.uint64(rank * S))
+        l_betas, l_ign, l_par, l_index = w.betas, w.ignitions, w.sim_param, np.arange(S)
+        if rank == 0:
+            assert (seeds_np == w.seeds).all()
+    S_all, S = S, int(len(l_index))                      # S = sims of this rank from here on
+    S_pad = (S_all + world - 1) // world if strong else S          # all_gather needs equal shards
 
     L = lf.fire_landscape_create(dev(ls["veg"]), dev(ls["slope"]), dev(ls["aspect"]), dev(ls["wind"]))
     H, Ww = L.H, L.Ww
-    if os.environ.get("FIRE_GEOM"):                      # tuning runs only: "threads,ctas_per_sm"
-        th, per = (int(v) for v in os.environ["FIRE_GEOM"].split(","))
-        lf.fire_set_launch_geometry(L, th, per)
-    if os.environ.get("FIRE_LIST"):                      # tuning runs only: "shared_entries,total_entries"
-        a, b = (int(v) for v in os.environ["FIRE_LIST"].split(","))
-        lf.fire_set_list_capacity(L, a, b)
-    if os.environ.get("FIRE_SCHEDULE"):
-        lf.fire_set_schedule(L, int(os.environ["FIRE_SCHEDULE"]))
     d_beta_ref = dev(w.ref_beta[None, :])
-    d_beta = dev(w.betas)
-    d_ign, d_par, d_seed, d_ids = dev(w.ignitions), dev(w.sim_param), dev(seeds_np), dev(sim_ids_np)
+    d_beta = dev(l_betas)
+    d_ign, d_par, d_seed, d_ids = dev(l_ign), dev(l_par), dev(seeds_np), dev(sim_ids_np)
     # the reference burnt map A: its own simulation from the stored vector, ignition and seed
     ref = torch.empty((1, H, Ww), dtype=torch.int32, device="cuda")
     lf.fire_params_upload(L, d_beta_ref)
@@ -236,9 +255,10 @@ def run_ours(args) -> None:
     burned = torch.empty((S, H, Ww), dtype=torch.int32, device="cuda")
     steps_out = torch.empty((S,), dtype=torch.int32, device="cuda")
     trials_out = torch.empty((S,), dtype=torch.int64, device="cuda")
-    score = torch.empty((S,), dtype=torch.float32, device="cuda")
+    score_buf = torch.full((max(S_pad, S),), float("nan"), dtype=torch.float32, device="cuda")
+    score = score_buf[:S]
     counts = torch.empty((S, 2), dtype=torch.int32, device="cuda")
-    gathered = torch.empty((world * S,), dtype=torch.float32, device="cuda") if world > 1 else None
+    gathered = torch.empty((world * max(S_pad, S),), dtype=torch.float32, device="cuda") if world > 1 else None
     if w.groups:
         G, R = w.groups
         g_sums = torch.empty((G, 2), dtype=torch.int64, device="cuda")
@@ -252,7 +272,7 @@ def run_ours(args) -> None:
         if w.groups:
             lf.fire_fitness_group_stats(counts, ref_area, G, R, g_sums, g_mv)
         if world > 1:
-            dist.all_gather_into_tensor(gathered, score)
+            dist.all_gather_into_tensor(gathered, score_buf)
 
     def fence():
         if world > 1:
@@ -278,13 +298,20 @@ def run_ours(args) -> None:
         generation()
     fence()
     trials_rank = int(trials_out.sum().item())
-    if rank == 0:
-        if trials_rank != golden["totals"]["trials"]:
-            raise RuntimeError(f"trial count {trials_rank} differs from the oracle's {golden['totals']['trials']}")
-        if not (steps_out.cpu().numpy().view(np.uint32) == np.array(golden["steps"], np.uint32)).all():
-            raise RuntimeError("steps differ from the oracle's stored values")
-        if not (counts.cpu().numpy().view(np.uint32)[:, 1] == np.array(golden["area"], np.uint32)).all():
-            raise RuntimeError("burned areas differ from the oracle's stored values")
+    bad = 0
+    if rank == 0 or strong:                              # these sims are sims of the stored config: every counter must match
+        if not (trials_out.cpu().numpy().view(np.uint64) == np.array(golden["trials"], np.uint64)[l_index]).all():
+            bad |= 1
+        if not (steps_out.cpu().numpy().view(np.uint32) == np.array(golden["steps"], np.uint32)[l_index]).all():
+            bad |= 2
+        if not (counts.cpu().numpy().view(np.uint32)[:, 1] == np.array(golden["area"], np.uint32)[l_index]).all():
+            bad |= 4
+    elif not (0.5 * golden["totals"]["trials"] < trials_rank < 2.0 * golden["totals"]["trials"]) or \
+            trials_rank == golden["totals"]["trials"]:   # other replicates of the same population: same law, other fires
+        bad |= 8
+    bad_any = sum_over_ranks(1 if bad else 0)
+    if bad_any:
+        raise RuntimeError(f"rank {rank}: counters differ from the oracle's stored values (flags {bad}; {bad_any} rank(s) failed)")
     trials_all = sum_over_ranks(trials_rank)
 
     # ---- device-resident timing: K steps between two events on the launching stream
@@ -322,7 +349,7 @@ def run_ours(args) -> None:
     clocks = sampler.stop() if rank == 0 else None
     ms_per_step = ms_total / args.steps
     value = trials_all * args.steps / (ms_total * 1e-3)
-    sims_per_s = world * S * args.steps / (ms_total * 1e-3)
+    sims_per_s = sum_over_ranks(S) * args.steps / (ms_total * 1e-3)
     phases = None
     if world == 1:
         phases = {"params_upload_ms": float(np.mean([e[0].elapsed_time(e[1]) for e in phase_ev])),
@@ -330,7 +357,7 @@ def run_ours(args) -> None:
                   "fitness_ms": float(np.mean([e[2].elapsed_time(e[3]) for e in phase_ev]))}
 
     # ---- end to end: host buffers in, scores out, every step (fire_generation_host synchronises)
-    h_beta, h_ign, h_par = pin(w.betas), pin(w.ignitions), pin(w.sim_param)
+    h_beta, h_ign, h_par = pin(l_betas), pin(l_ign), pin(l_par)
     h_seed, h_ids, h_ref = pin(seeds_np), pin(sim_ids_np), pin(ref[0].cpu().numpy())
     h_score = torch.empty(S, dtype=torch.float32).pin_memory()
     h_counts = torch.empty((S, 2), dtype=torch.int32).pin_memory()
@@ -340,7 +367,8 @@ def run_ours(args) -> None:
     def generation_host():
         lf.fire_generation_host(L, h_beta, h_ign, h_par, h_seed, h_ref, w.metric, h_score, h_counts, sim_ids=h_ids)
         if world > 1:
-            dist.all_gather_into_tensor(gathered, h_score.cuda(non_blocking=True))
+            score_buf[:S].copy_(h_score, non_blocking=True)
+            dist.all_gather_into_tensor(gathered, score_buf)
 
     generation_host()
     fence()
@@ -370,42 +398,48 @@ def run_ours(args) -> None:
     else:
         peak, peak_src = 6650.0, "B200_PROFILING.md fallback (of fallback)"
     plane_bytes = H * Ww * 4
-    alg_bytes = 32 * golden["totals"]["distinct"] + 2 * plane_bytes * S
+    alg_bytes = 32 * int(np.array(golden["distinct"], np.int64)[l_index].sum()) + 2 * plane_bytes * S
     k_ms = float(np.mean(prop_ms)) if prop_ms else float("nan")
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": "fire_propagate_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg) if world == 1 else None,
+                "traffic_source": NCU_TRAFFIC_SOURCE.get(cfg) if world == 1 else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms, "launches_timed": len(prop_ms),
                 "share_of_step": k_ms / ms_per_step,
-                "philox_calls_per_s": golden["totals"]["trials"] / (k_ms * 1e-3)}
+                "philox_calls_per_s": trials_rank / (k_ms * 1e-3)}
     # second ceiling: the kernel is issue-bound, not HBM-bound.  Algorithmic integer work = one
     # Philox4x32-10 call per trial = 20 wide multiplies + 20 three-input xors = 40 lane operations; peak = SMs x 4 schedulers
     # x 32 lanes x max SM clock, one instruction per scheduler per clock.
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     sm_clock_hz = 1e6 * float((clocks or {}).get("sm_max_mhz") or 1965.0)
     alu_peak = sm_count * 4 * 32 * sm_clock_hz
-    alu_ach = 40.0 * golden["totals"]["trials"] / (k_ms * 1e-3)
+    alu_ach = 40.0 * trials_rank / (k_ms * 1e-3)
     roofline["alu"] = {"bound": "alu", "achieved": alu_ach / 1e12, "peak": alu_peak / 1e12, "unit": "Tera lane-ops/s",
                        "frac": alu_ach / alu_peak, "note": "40 lane-ops per trial (Philox4x32-10) / issue peak"}
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample of the same workload
     cpu = None
     if world == 1 and not args.no_cpu:
-        wq, n = oracle_sample(cfg, sample_budget(cfg))
-        tr, dt, threads = time_oracle(wq, n)
+        wq, idx = oracle_sample(cfg, sample_budget(cfg))
+        tr, dt, threads = time_oracle(wq, idx)
+        idx1 = idx[:: max(1, threads)]                    # the single-thread figure on a 1/threads sub-sample: the same wall time
+        tr1, dt1, _ = time_oracle(wq, idx1, nthreads=1)
         cpu = {"value": tr / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": f"first {n} of {wq.S} simulations of {wq.name} (+ Eq. 2 counts), {dt:.1f} s",
-               "sims_per_s": n / dt}
+               "sample": sample_text(wq, idx) + f", {dt:.1f} s", "sims_per_s": len(idx) / dt,
+               "single_thread": {"value": tr1 / dt1, "unit": UNIT, "cores": 1, "sims": int(len(idx1)), "seconds": dt1}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong" if strong else "weak", "vs_baseline": None,
         "dtype": "u32", "data": "synthetic",
         "config": {"workload": w.name, "lattice": f"{L.W}x{L.H}", "param_vectors": P, "sims_per_gpu": S,
+                   "param_vectors_per_gpu": int(l_betas.shape[0]), "comm_nranks": world,
                    "step": "params_upload + simulate_batch + fitness (one GA generation)",
                    "l2": "inputs larger than L2: the threshold table is "
                          f"{P * L.W * L.H * 32 / 2**30:.2f} GiB and is rewritten every step",
-                   "parallelism": f"sims sharded over {world} GPU(s), landscape replicated"},
+                   "parallelism": (f"one generation partitioned by parameter vector over {world} GPU(s): each builds P/N of the table"
+                                   if strong else f"one generation of S sims per GPU on {world} GPU(s) (replicates r*S..), no data-path collective")
+                                  + ", landscape replicated, one all-gather of the scores per step"},
         "sims_per_s": sims_per_s, "trials_per_step": trials_all, "phases_ms": phases,
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -428,6 +462,8 @@ def main() -> None:
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--cfg", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one generation of S sims per GPU (default); strong = ONE generation partitioned by parameter vector")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -26,6 +26,16 @@
  * done.  The handle owns covariates, thresholds, scratch planes and queues.
  * Asynchrony: every call only enqueues work on `stream` unless stated otherwise; outputs are valid
  * once the caller has synchronised the stream.  A handle must not be used from two streams at once.
+ * The one exception to "only enqueues": the handle's internal buffers are grow-only, and a call that has to
+ * GROW one (a larger P in fire_params_upload, a larger S in fire_simulate_batch / fire_fitness /
+ * fire_generation_host than any call before on this handle) first waits for `stream` (cudaStreamSynchronize),
+ * because work already enqueued may still use the old buffer.  Repeating a call with sizes the handle has
+ * already seen never synchronises.
+ * Limits (violations return FIRE_EINVAL before anything is enqueued; the handle stays usable):
+ *   1 <= W, H <= 8192;  P * W * H < 2^32 (threshold sectors are addressed by 32-bit indices: 137 GB of table);
+ *   S * ceil(W/8) * ceil(H/8) < 2^31 per fire_simulate_batch call (state planes are addressed by 32-bit tile
+ *   offsets; 2^30 when the two-plane kernel family is selected): 131,071 simulations on a 1024 x 1024 lattice,
+ *   8,191 on 4096 x 4096 -- split larger batches over several calls, using sim_ids to keep the random streams.
  * Errors: 0 on success, a negative FIRE_E* code otherwise.  The library never throws, aborts or
  * prints.  Faults only the device can see (ignition outside the lattice or on a non-burnable
  * cell, sim_param outside [0, P)) are not errors: that simulation burns nothing, steps = 0 (R-12).
@@ -41,7 +51,7 @@ extern "C" {
 #endif
 
 #define FIRE_OK       0
-#define FIRE_EINVAL  (-1)   /* null pointer, non-positive size, R < 2, lattice larger than 8192 x 8192 */
+#define FIRE_EINVAL  (-1)   /* null pointer, non-positive size, R < 2, a limit listed above exceeded */
 #define FIRE_ENOMEM  (-2)   /* device allocation failed */
 #define FIRE_ESTATE  (-3)   /* simulate before fire_params_upload, p out of range in download */
 #define FIRE_ECUDA   (-4)   /* a CUDA call failed (sticky), or no CUDA device */
@@ -122,8 +132,8 @@ int fire_set_profiling(fire_landscape* L, int32_t enabled);
 int fire_profile_read(fire_landscape* L, float* ms_host, int32_t max_entries, int32_t* n_out);
 
 /* Tuning knob (tests use it to show results do not depend on launch geometry, pin P-9):
- * threads per CTA of the propagation kernel (multiple of 32, 64..1024; 0 = default) and CTAs per SM
- * (0 = default). */
+ * threads per CTA of the propagation kernel (multiple of 32, 32..1024; 0 = default) and CTAs per SM
+ * (0..32; 0 = default). */
 int fire_set_launch_geometry(fire_landscape* L, int32_t threads_per_cta, int32_t ctas_per_sm);
 
 /* Test hook (pin P-9): capacity, in cells, of the per-CTA frontier list of the propagation kernel:

@@ -121,8 +121,13 @@ fire_group_stats_kernel(const uint32_t* __restrict__ counts, uint32_t N, int G, 
     if (lane == 0) {
         sums[2 * g] = sx; sums[2 * g + 1] = sxx;
         const double mean = __ddiv_rn((double)sx, __dmul_rn((double)R, (double)N));
-        const unsigned long long num = (unsigned long long)R * sxx - sx * sx;               // exact, >= 0
-        double var = __ddiv_rn((double)num, (double)((unsigned long long)R * (unsigned long long)(R - 1)));
+        // numerator R sum x^2 - (sum x)^2 >= 0 as a 128-bit integer (x reaches 2 W H: the 64-bit expression wraps from
+        // R = 33 on an 8192 x 8192 lattice); one conversion to double when it fits 64 bits (always, at BASELINE's sizes)
+        const unsigned long long a_lo = (unsigned long long)R * sxx, a_hi = __umul64hi((unsigned long long)R, sxx);
+        const unsigned long long b_lo = sx * sx, b_hi = __umul64hi(sx, sx);
+        const unsigned long long n_lo = a_lo - b_lo, n_hi = a_hi - b_hi - (a_lo < b_lo ? 1ull : 0ull);
+        const double num = n_hi == 0ull ? (double)n_lo : __fma_rn((double)n_hi, 18446744073709551616.0, (double)n_lo);
+        double var = __ddiv_rn(num, (double)((unsigned long long)R * (unsigned long long)(R - 1)));
         var = __ddiv_rn(var, __dmul_rn((double)N, (double)N));
         mean_var[2 * g] = mean; mean_var[2 * g + 1] = var;
     }

@@ -73,11 +73,7 @@ struct thr_sector { uint4 a, b; };     // a = directions 0..3, b = directions 4.
 __device__ __forceinline__ thr_sector ldg_thr(const uint4* p)
 {
     thr_sector v;
-#if defined(FIRE_THR_L1)
-    asm volatile("ld.global.nc.L2::128B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-#else
     asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
-#endif
                  : "=r"(v.a.x), "=r"(v.a.y), "=r"(v.a.z), "=r"(v.a.w), "=r"(v.b.x), "=r"(v.b.y), "=r"(v.b.z), "=r"(v.b.w) : "l"(p));
     return v;
 }
@@ -308,9 +304,6 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
         pt.old[u] = 0u;
         if (fire_trial(rnd, T[u])) {
             pt.old[u] = atomicAnd(reinterpret_cast<uint32_t*>(const_cast<uint64_t*>(c.tiles)) + (c.plane_w2 + widx), ~(1u << pt.bit[u]));
-#ifdef FIRE_PREFETCH_THR
-            asm volatile("prefetch.global.L2 [%0];" :: "l"(c.thr4 + (size_t)(c.thr_sec + cell) * 2));
-#endif
         }
     }
 }
@@ -417,9 +410,6 @@ fire_propagate_kernel(const prop_params prm)
         __syncthreads();
         const uint32_t s = s_sim;
         if (s == 0xFFFFFFFFu) break;
-#ifdef FIRE_TRACE
-        unsigned long long trace_t0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t0));
-#endif
 
         const int p = prm.sim_param[s];
         const int ix = prm.ignitions[2 * s], iy = prm.ignitions[2 * s + 1];
@@ -523,10 +513,6 @@ fire_propagate_kernel(const prop_params prm)
             } else {
                 if (prm.out_steps) prm.out_steps[s] = t;
                 if (prm.out_trials) prm.out_trials[s] = s_trials;
-#ifdef FIRE_TRACE   // diagnostic build only: out_trials = (start us << 32) | duration us of this simulation, for schedule plots
-                unsigned long long trace_t1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t1));
-                if (prm.out_trials) prm.out_trials[s] = (((trace_t0 / 1000ull) & 0xFFFFFFFFull) << 32) | (((trace_t1 - trace_t0) / 1000ull) & 0xFFFFFFFFull);
-#endif
             }
         }
     }
@@ -621,9 +607,6 @@ fire_propagate_async_kernel(const prop_params prm)
         __syncthreads();
         const uint32_t s = s_sim;
         if (s == 0xFFFFFFFFu) break;
-#ifdef FIRE_TRACE
-        unsigned long long trace_t0; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t0));
-#endif
         const int p = prm.sim_param[s];
         const int ix = prm.ignitions[2 * s], iy = prm.ignitions[2 * s + 1];
         const uint64_t seed = prm.seeds[s];
@@ -757,10 +740,6 @@ fire_propagate_async_kernel(const prop_params prm)
                 prm.plane_sel[s] = t & 1u;                         // the plane that holds the final state
                 if (prm.out_steps) prm.out_steps[s] = t;
                 if (prm.out_trials) prm.out_trials[s] = s_trials;
-#ifdef FIRE_TRACE
-                unsigned long long trace_t1; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(trace_t1));
-                if (prm.out_trials) prm.out_trials[s] = (((trace_t0 / 1000ull) & 0xFFFFFFFFull) << 32) | (((trace_t1 - trace_t0) / 1000ull) & 0xFFFFFFFFull);
-#endif
             }
         }
     }

@@ -165,3 +165,47 @@ def shard_sims(S: int, rank: int, world: int) -> slice:
     base, rem = divmod(S, world)
     lo = rank * base + min(rank, rem)
     return slice(lo, lo + base + (1 if rank < rem else 0))
+
+
+@dataclass
+class ParamShard:
+    """What rank ``rank`` of ``world`` runs when a generation is partitioned BY PARAMETER VECTOR (PAPER.md:117:
+    individuals are independent): the rank uploads only `betas` (so it builds P_local / P of the threshold table), simulates
+    the sims at positions `index` of the batch with `sim_param` re-based to its slice and `sim_ids` = their global batch
+    positions (the `sim` field of the random-number key, so every fire is the one the full batch would produce)."""
+    p_lo: int
+    p_hi: int
+    betas: np.ndarray          # f32 [P_local][5]
+    index: np.ndarray          # i64 [S_local]  positions in the full batch, ascending
+    sim_param: np.ndarray      # i32 [S_local]  in [0, P_local)
+    sim_ids: np.ndarray        # i32 [S_local]  = index
+    ignitions: np.ndarray      # i32 [S_local][2]
+    seeds: np.ndarray          # u64 [S_local]
+
+
+def shard_by_param(w: Workload, rank: int, world: int) -> ParamShard:
+    """Contiguous, near-equal slices of the parameter-vector axis; a sim goes where its vector goes.  Sims whose `sim_param`
+    is outside [0, P) (R-12: they burn nothing) go to rank 0, which keeps them invalid (index P_local)."""
+    sl = shard_sims(w.P, rank, world)
+    sp = np.asarray(w.sim_param, np.int64)
+    mine = (sp >= sl.start) & (sp < sl.stop)
+    if rank == 0:
+        mine |= (sp < 0) | (sp >= w.P)
+    index = np.flatnonzero(mine)
+    local = sp[index] - sl.start
+    local[(sp[index] < 0) | (sp[index] >= w.P)] = sl.stop - sl.start          # stays out of range
+    return ParamShard(p_lo=sl.start, p_hi=sl.stop, betas=np.ascontiguousarray(w.betas[sl]), index=index,
+                      sim_param=local.astype(np.int32), sim_ids=index.astype(np.int32),
+                      ignitions=np.ascontiguousarray(w.ignitions[index]), seeds=np.ascontiguousarray(w.seeds[index]))
+
+
+def merge_param_shards(parts: list, values: list, S: int) -> np.ndarray:
+    """Per-shard result vectors (one entry per local sim) back into batch order."""
+    out = np.empty((S,) + tuple(np.asarray(values[0]).shape[1:]), dtype=np.asarray(values[0]).dtype)
+    seen = np.zeros(S, bool)
+    for sh, v in zip(parts, values):
+        out[sh.index] = np.asarray(v)[: len(sh.index)]
+        seen[sh.index] = True
+    if not seen.all():
+        raise ValueError("shards do not cover the batch")
+    return out

@@ -43,6 +43,18 @@ def test_binding_covers_the_header_and_loads(lib_path):
     assert lf.error_string(lf.FIRE_OK) == "ok" and "invalid" in lf.error_string(lf.FIRE_EINVAL)
 
 
+def test_header_is_valid_c99_and_prototypes_match(tmp_path):
+    """include/fire.h through a C compiler (not a regex): tests/c/abi_c99.c includes it, assigns every declared call to a
+    function pointer of the documented prototype and names every error / metric code."""
+    src = ROOT / "tests" / "c" / "abi_c99.c"
+    res = subprocess.run(["gcc", "-std=c99", "-pedantic", "-Wall", "-Wextra", "-Werror", "-I", str(ROOT / "include"),
+                          "-c", str(src), "-o", str(tmp_path / "abi_c99.o")], capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
+    text = src.read_text()
+    for name in declared_symbols():
+        assert re.search(rf"=\s*{name}\s*;", text), f"{name} is not referenced by tests/c/abi_c99.c"
+
+
 def test_library_is_built_for_sm_100a(lib_path):
     out = subprocess.run(["cuobjdump", "-lelf", str(lib_path)], capture_output=True, text=True).stdout
     assert "sm_100a" in out

@@ -53,6 +53,19 @@ def _rank_main(rank: int, world: int, port: int, out_dir: str) -> None:
     dist.all_reduce(trials, op=dist.ReduceOp.SUM)
     t = torch.tensor([float(rank + 1)], dtype=torch.float64)           # "max over ranks" timing reduction
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    # ---- the same generation partitioned BY PARAMETER VECTOR: every rank holds only its P / world vectors
+    sh = wl.shard_by_param(w, rank, world)
+    assert sh.betas.shape[0] == w.P // world and sh.sim_param.max() < sh.betas.shape[0]
+    rp = orc.simulate_batch(Lo, sh.betas, sh.ignitions, sh.sim_param, sh.seeds, sim_index=sh.sim_ids, nthreads=1)
+    _, score_p, _ = orc.fitness(ref, rp["burned"], Lo.W, w.metric)
+    mine_p = torch.full((per,), float("nan"), dtype=torch.float32)
+    mine_p[: len(score_p)] = torch.from_numpy(score_p)
+    gathered_p = torch.empty((world * per,), dtype=torch.float32)
+    dist.all_gather_into_tensor(gathered_p, mine_p)
+    if rank == 0:
+        shards = [wl.shard_by_param(w, k, world) for k in range(world)]
+        vals = [gathered_p[k * per: k * per + len(shards[k].index)].numpy() for k in range(world)]
+        np.save(os.path.join(out_dir, "scores_by_param.npy"), wl.merge_param_shards(shards, vals, w.S))
     if rank == 0:
         parts = [gathered[k * per: k * per + (wl.shard_sims(w.S, k, world).stop - wl.shard_sims(w.S, k, world).start)]
                  for k in range(world)]
@@ -81,6 +94,32 @@ def test_two_rank_sharding_reproduces_the_full_batch(orc, tmp_path):
     assert np.array_equal(got.view(np.uint32), score.view(np.uint32))
     assert int(np.load(tmp_path / "trials.npy")[0]) == int(full["trials"].sum())
     assert float(np.load(tmp_path / "tmax.npy")[0]) == float(world)
+    got_p = np.load(tmp_path / "scores_by_param.npy")
+    assert np.array_equal(got_p.view(np.uint32), score.view(np.uint32))          # batch order, bit for bit
+
+
+def test_param_shards_partition_vectors_and_sims():
+    from paper_1701_03549_b200 import workloads as wl
+    for cfg in (1, 2):
+        w = wl.load_workload(cfg)
+        for world in (1, 2, 3, 8):
+            shards = [wl.shard_by_param(w, r, world) for r in range(world)]
+            assert shards[0].p_lo == 0 and shards[-1].p_hi == w.P
+            assert all(a.p_hi == b.p_lo for a, b in zip(shards, shards[1:]))
+            assert max(s.betas.shape[0] for s in shards) - min(s.betas.shape[0] for s in shards) <= 1
+            allidx = np.concatenate([s.index for s in shards])
+            assert np.array_equal(np.sort(allidx), np.arange(w.S))
+            for s in shards:
+                assert np.array_equal(w.betas[s.p_lo + s.sim_param], w.betas[w.sim_param[s.index]])   # same vector, re-based index
+                assert np.array_equal(s.sim_ids, s.index.astype(np.int32))
+            back = wl.merge_param_shards(shards, [w.seeds[s.index] for s in shards], w.S)
+            assert np.array_equal(back, w.seeds)
+    # an out-of-range vector index stays invalid on rank 0
+    w = wl.load_workload(1)
+    w.sim_param = w.sim_param.copy(); w.sim_param[5] = -3; w.sim_param[9] = w.P + 7
+    sh0 = wl.shard_by_param(w, 0, 2)
+    assert 5 in sh0.index and 9 in sh0.index
+    assert (sh0.sim_param[np.isin(sh0.index, [5, 9])] == sh0.betas.shape[0]).all()
 
 
 def test_shards_are_contiguous_and_cover_the_batch():
