@@ -149,7 +149,9 @@ int fire_set_schedule(fire_landscape* L, int32_t mode);
 
 /* Test hook (pin P-9): which propagation kernel fire_simulate_batch launches.  0 = automatic (by batch size),
  * 1 = two-phase kernel (one CTA per simulation, one state plane, two block barriers per step), 2 = asynchronous-warp
- * kernel (one CTA per simulation, two state planes, one block barrier per step).  Results never depend on it. */
+ * kernel (one CTA per simulation, two state planes, one block barrier per step), 3 / 4 = the asynchronous-warp kernel as
+ * thread-block clusters of 2 / 4 CTAs per simulation (one cluster barrier per step; frontier lists read through
+ * distributed shared memory).  Results never depend on it. */
 int fire_set_kernel(fire_landscape* L, int32_t family);
 
 const char* fire_error_string(int code);

@@ -572,13 +572,41 @@ __device__ __forceinline__ void trials_issue_ring(const step_ctx& c, const philo
 // ------------------------------------------------------------------------------------------------
 constexpr uint32_t kRingEntries = 512;             // per warp, 8 B each: one cell unit adds at most 256 trials to at most 31 left over
 
-template <int kMaxThreads, int kMinCtas>
+// With kCluster the kernel is launched as thread-block CLUSTERS of 2 or 4 CTAs (sm_90+), one cluster per simulation, for
+// batches smaller than the GPU (config 5: 64 simulations of 4096 x 4096 on 148 SMs).  The state planes are in global memory
+// (L2) and so are shared by construction; every CTA keeps the frontier list of the cells IT ignited in its own shared memory
+// and the other CTAs of the cluster read it through distributed shared memory: of every list, CTA r runs the units
+// u = (r + owner) mod size, so the work of a step is dealt evenly whoever owns the cells.  One cluster barrier per step.
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cluster_nctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cluster_map(uint32_t addr, uint32_t rank)
+{
+    uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank)); return r;
+}
+__device__ __forceinline__ uint32_t ld_cluster32(uint32_t addr)
+{
+    uint32_t v; asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
+}
+__device__ __forceinline__ void st_cluster32(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.shared::cluster.u32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
+}
+template <bool kCluster>
+__device__ __forceinline__ void team_sync()
+{
+    if (kCluster) asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    else __syncthreads();
+}
+constexpr int kMaxClusterSize = 4;
+
+template <int kMaxThreads, int kMinCtas, bool kCluster>
 __global__ void __launch_bounds__(kMaxThreads, kMinCtas)
 fire_propagate_async_kernel(const prop_params prm)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     const int tid = threadIdx.x;
     const uint32_t warp = (uint32_t)tid >> 5, nwarps = blockDim.x >> 5;
+    const uint32_t crank = kCluster ? cluster_ctarank() : 0u, csize = kCluster ? cluster_nctarank() : 1u;
     // shared layout: per-warp trial rings, frontier list 0, frontier list 1
     uint32_t ring_addr = (uint32_t)__cvta_generic_to_shared(smem) + warp * (kRingEntries * 8u);
     asm volatile("" : "+r"(ring_addr));
@@ -600,11 +628,17 @@ fire_propagate_async_kernel(const prop_params prm)
     c.over = cntA_addr + 12u;
     c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
     const size_t nt = (size_t)c.Tw * c.Th;
+    const uint32_t sim_addr = cntA_addr + 16u;
+    const uint32_t trials_addr = (uint32_t)__cvta_generic_to_shared(&s_trials);
 
     for (;;) {
-        __syncthreads();
-        if (tid == 0) s_sim = next_simulation(prm);
-        __syncthreads();
+        team_sync<kCluster>();                 // the previous simulation's last (remote) reads of s_* are done
+        if (tid == 0 && crank == 0) {
+            const uint32_t nxt = next_simulation(prm);
+            if (kCluster) { for (uint32_t j = 0; j < csize; ++j) st_cluster32(cluster_map(sim_addr, j), nxt); }
+            else s_sim = nxt;
+        }
+        team_sync<kCluster>();
         const uint32_t s = s_sim;
         if (s == 0xFFFFFFFFu) break;
         const int p = prm.sim_param[s];
@@ -620,20 +654,25 @@ fire_propagate_async_kernel(const prop_params prm)
         const uint32_t bh = __umulhi(sim, kM1), bl = sim * kM1;
 
         if (tid == 0) {
-            s_cntA[0] = valid ? 1u : 0u; s_cntA[1] = 0u; s_cntA[2] = 0u; s_over = 0u; s_trials = 0ull;
-            if (valid) {
+            const bool seeded = valid && crank == 0u;              // the ignition cell belongs to the first CTA of the cluster
+            s_cntA[0] = seeded ? 1u : 0u; s_cntA[1] = 0u; s_cntA[2] = 0u; s_over = 0u; s_trials = 0ull;
+            if (seeded) {
                 const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
                 if (prm.capA_s > 0) sts32(as_addr0, e0); else prm.spill[ag_off0] = e0;
                 // the ignition is burnt at t = 0: cleared in plane 0 (read by step 0); plane 1 is caught up by step 0 itself
                 atomicAnd(reinterpret_cast<uint32_t*>(plane0) + (((size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
         }
-        __syncthreads();
+        team_sync<kCluster>();
 
         uint32_t t = 0, my_trials = 0;
-        c.nA = valid ? 1u : 0u;
+        uint32_t nA_of[kMaxClusterSize];                           // length of every CTA's current list; [0] is the only one without clusters
+#pragma unroll
+        for (int j = 0; j < kMaxClusterSize; ++j) nA_of[j] = 0u;
+        nA_of[0] = valid ? 1u : 0u;
+        uint32_t nA_total = nA_of[0];
         bool over = false;
-        while (c.nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
+        while (nA_total > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
             const uint32_t par = t & 1u;
             c.ac_addr = par ? as_addr1 : as_addr0; c.an_addr = par ? as_addr0 : as_addr1;
             c.ac_off = par ? ag_off1 : ag_off0; c.an_off = par ? ag_off0 : ag_off1;
@@ -651,13 +690,25 @@ fire_propagate_async_kernel(const prop_params prm)
 
             uint32_t head = 0, fill = 0;                           // this warp's ring: entries [head, head + fill) mod kRingEntries
             pending_trials prev; bool have = false;
-            const uint32_t nU = (c.nA + 31u) >> 5;
-            for (uint32_t u = warp; u < nU; u += nwarps) {
+#pragma unroll 1
+            for (uint32_t j = 0; j < csize; ++j) {                 // the list of every CTA of the cluster (own list only without clusters)
+            const uint32_t nA_j = kCluster ? nA_of[j] : nA_of[0];
+            c.nA = nA_j;
+            const uint32_t nU = (nA_j + 31u) >> 5;
+            // where list j lives: the owner's shared memory (through the cluster window if it is not this CTA) and its global spill
+            const bool own = !kCluster || j == crank;
+            const uint32_t lst_addr = own ? c.ac_addr : cluster_map(c.ac_addr, j);
+            const uint32_t lst_off = kCluster ? (uint32_t)((size_t)(blockIdx.x - crank + j) * spill_per_cta) + (c.ac_off - qg_off) : c.ac_off;
+            const uint32_t u_first = kCluster ? ((crank + csize - (j % csize)) % csize) + csize * warp : warp;
+            const uint32_t u_step = kCluster ? csize * nwarps : nwarps;
+            for (uint32_t u = u_first; u < nU; u += u_step) {
                 // ---- one unit of 32 burning cells: window, thresholds, catch-up, trials appended to the ring
                 uint32_t i = u * 32u + c.lane;
                 const bool live = i < c.nA;
                 i = live ? i : c.nA - 1u;
-                const uint32_t e = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.spill + (c.ac_off + (i - c.capA_s)));
+                uint32_t e;
+                if (i < c.capA_s) e = own ? lds32(lst_addr + 4u * i) : ld_cluster32(lst_addr + 4u * i);
+                else e = __ldcg(c.spill + (lst_off + (i - c.capA_s)));
                 const uint32_t x = e & 0xFFFFu, y = e >> 16;
                 const uint32_t tx0 = x >> 3, ty0 = y >> 3, bx = x & 7u, by = y & 7u;
                 const uint32_t tidx = ty0 * c.Tw + tx0;
@@ -715,6 +766,7 @@ fire_propagate_async_kernel(const prop_params prm)
                 fill += total;
                 __syncwarp();
             }
+            }
             // ---- the rest of the ring, last unit possibly partial
             while (fill > 0u) {
                 const uint32_t n = fill < 64u ? fill : 64u;
@@ -725,25 +777,46 @@ fire_propagate_async_kernel(const prop_params prm)
                 head = (head + n) & (kRingEntries - 1u); fill -= n;
             }
             if (have) trials_resolve<2>(c, prev);
-            __syncthreads();
+            team_sync<kCluster>();
             ++t;
-            if (s_over) { over = true; break; }
-            c.nA = s_cntA[t % 3u];
+            if (kCluster) {                                        // every CTA reads every CTA's flags and counters: all take the same decisions
+                uint32_t ov[kMaxClusterSize];                      // all the remote loads first, then their uses: one round trip
+#pragma unroll
+                for (int j = 0; j < kMaxClusterSize; ++j) {
+                    ov[j] = 0u; nA_of[j] = 0u;
+                    if ((uint32_t)j < csize) {
+                        ov[j] = ld_cluster32(cluster_map(c.over, (uint32_t)j));
+                        nA_of[j] = ld_cluster32(cluster_map(cntA_addr + 4u * (t % 3u), (uint32_t)j));
+                    }
+                }
+                const uint32_t any_over = ov[0] | ov[1] | ov[2] | ov[3];
+                nA_total = nA_of[0] + nA_of[1] + nA_of[2] + nA_of[3];
+                if (any_over) { over = true; break; }
+            } else {
+                if (s_over) { over = true; break; }
+                nA_of[0] = s_cntA[t % 3u];
+                nA_total = nA_of[0];
+            }
         }
 
         if (my_trials) atomicAdd(&s_trials, (unsigned long long)my_trials);
-        __syncthreads();
-        if (tid == 0) {
+        team_sync<kCluster>();
+        if (tid == 0 && crank == 0u) {
             if (over) {
                 prm.rescue_list[atomicAdd(prm.work_counter + 1, 1u)] = s;
             } else {
+                unsigned long long trials = s_trials;
+                if (kCluster)
+                    for (uint32_t j = 1; j < csize; ++j)
+                        trials += ((unsigned long long)ld_cluster32(cluster_map(trials_addr + 4u, j)) << 32) | ld_cluster32(cluster_map(trials_addr, j));
                 prm.plane_sel[s] = t & 1u;                         // the plane that holds the final state
                 if (prm.out_steps) prm.out_steps[s] = t;
-                if (prm.out_trials) prm.out_trials[s] = s_trials;
+                if (prm.out_trials) prm.out_trials[s] = trials;
             }
         }
     }
 }
+
 
 // ------------------------------------------------------------------------------------------------
 // Plane set-up and tear-down around the fast kernel (pure streams).
@@ -987,7 +1060,7 @@ extern "C" int fire_set_schedule(fire_landscape* L, int32_t mode)
 
 extern "C" int fire_set_kernel(fire_landscape* L, int32_t family)
 {
-    if (L == nullptr || family < 0 || family > 2) return FIRE_EINVAL;
+    if (L == nullptr || family < 0 || family > 4) return FIRE_EINVAL;
     L->kernel_family = family;
     return FIRE_OK;
 }
@@ -1017,11 +1090,16 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         if (threads == 0) threads = 256;
         if (per_sm == 0) per_sm = (1024 / threads) > 0 ? (1024 / threads) : 1;
     }
-    const int grid = (int)((long long)S < (long long)L->num_sms * per_sm ? S : L->num_sms * per_sm);
     // kernel family (fire_set_kernel): 1 = two-phase kernel (one state plane, two block barriers per step), 2 = asynchronous-warp
-    // kernel (two state planes, one barrier per step, per-warp trial rings); 0 = the two-phase kernel for batches that fill the GPU
-    // with 256-thread CTAs, the asynchronous-warp kernel for small batches of large fires (wide CTAs, long fronts)
-    const bool async = L->kernel_family == 2 || (L->kernel_family == 0 && threads >= 512 && L->threads_per_cta == 0);
+    // kernel (two state planes, one barrier per step, per-warp trial rings), 3 / 4 = the same as thread-block clusters of 2 / 4
+    // CTAs per simulation; 0 = the two-phase kernel for batches that fill the GPU with 256-thread CTAs, the asynchronous-warp
+    // kernel for small batches of large fires (wide CTAs, long fronts), as clusters when the batch is smaller than half the GPU
+    const bool async = L->kernel_family >= 2 || (L->kernel_family == 0 && threads >= 512 && L->threads_per_cta == 0);
+    int cluster = L->kernel_family == 3 ? 2 : (L->kernel_family == 4 ? 4 : 1);
+    if (L->kernel_family == 0 && async && threads == 1024)
+        cluster = (long long)S * 4 <= L->num_sms ? 4 : ((long long)S * 2 <= L->num_sms ? 2 : 1);
+    const long long resident = (long long)L->num_sms * per_sm / cluster;         // simulations in flight
+    const int grid = (int)((long long)S < resident ? S : (resident < 1 ? 1 : resident)) * cluster;
     const int planes = async ? 2 : 1;
     prop_params prm;
     uint32_t capA = L->list_capacity ? (uint32_t)L->list_capacity : 0u;
@@ -1096,7 +1174,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
 
     // ---- launch order: largest expected fires first (only matters when there are more simulations than resident ones)
     prm.order = nullptr;
-    if (S > grid && L->param_mean != nullptr && L->schedule == 0) {
+    if (S > grid / cluster && L->param_mean != nullptr && L->schedule == 0) {
         fire_order_kernel<<<1, 1024, 0, st>>>(sim_param, L->param_mean, S, L->P, 1.0f / ((float)L->cells * 8.0f), L->order);
         FIRE_CUDA_TRY(L, cudaGetLastError());
         L->launches += 1;
@@ -1117,7 +1195,8 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     if (async) FIRE_CUDA_TRY(L, cudaMemsetAsync(L->status + S, 0, (size_t)S * 4, st));
     // instantiations differ in their register budget only (threads <= kMaxThreads is the one hard constraint)
     void (*kernel)(const prop_params) = nullptr;
-    if (async) kernel = threads <= 256 ? fire_propagate_async_kernel<256, 4> : (threads <= 512 ? fire_propagate_async_kernel<512, 2> : fire_propagate_async_kernel<1024, 1>);
+    if (async && cluster > 1) kernel = threads <= 256 ? fire_propagate_async_kernel<256, 4, true> : (threads <= 512 ? fire_propagate_async_kernel<512, 2, true> : fire_propagate_async_kernel<1024, 1, true>);
+    else if (async) kernel = threads <= 256 ? fire_propagate_async_kernel<256, 4, false> : (threads <= 512 ? fire_propagate_async_kernel<512, 2, false> : fire_propagate_async_kernel<1024, 1, false>);
     else kernel = threads <= 256 ? (per_sm <= 4 ? fire_propagate_kernel<256, 4, 2, 4> : fire_propagate_kernel<256, 8, 1, 2>)
                                  : (threads <= 512 ? fire_propagate_kernel<512, 2, 2, 4> : fire_propagate_kernel<1024, 1, 2, 4>);
     if (smem + 1024 > 48 * 1024)                     // dynamic + static shared memory beyond the default limit
@@ -1129,7 +1208,17 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     }
     const bool prof = L->prof_enabled && L->prof_count < 64;
     if (prof) FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count], st));
-    kernel<<<grid, threads, smem, st>>>(prm);
+    if (cluster > 1) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)cluster; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        FIRE_CUDA_TRY(L, cudaLaunchKernelEx(&cfg, kernel, prm));
+    } else {
+        kernel<<<grid, threads, smem, st>>>(prm);
+    }
     FIRE_CUDA_TRY(L, cudaGetLastError());
     if (prof) { FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count + 1], st)); L->prof_count += 1; }
     {

@@ -271,14 +271,16 @@ def test_results_do_not_depend_on_launch_geometry_or_list_capacity(request):
     again = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
     assert (base["burned"] == again["burned"]).all()
     # (threads per CTA, CTAs per SM, shared list entries, total list entries, launch order, kernel family)
-    # family 0 = automatic, 1 = two-phase kernel, 2 = asynchronous-warp kernel
+    # family 0 = automatic, 1 = two-phase kernel, 2 = asynchronous-warp kernel, 3 / 4 = the latter as clusters of 2 / 4 CTAs
     for threads, per_sm, shared, total, order, family in [
             (32, 1, 0, 0, 0, 0), (64, 8, 0, 0, 1, 0), (128, 2, 0, 0, 0, 0), (512, 1, 0, 0, 0, 1), (1024, 1, 0, 0, 1, 1),
             (256, 4, 16, 0, 0, 0), (256, 4, 5, 4096, 1, 0), (96, 3, 1, 0, 0, 0), (256, 4, 8, 8, 0, 0),
             (128, 4, 64, 100, 1, 0), (256, 2, 0, 1, 0, 0), (256, 5, 0, 0, 0, 0), (256, 6, 0, 0, 1, 0),
             (256, 8, 768, 0, 0, 0), (128, 1, 0, 0, 1, 0), (128, 16, 0, 0, 0, 1), (0, 0, 0, 0, 0, 1),
             (256, 4, 0, 0, 0, 2), (32, 2, 0, 0, 1, 2), (1024, 1, 0, 0, 0, 2), (512, 2, 16, 0, 0, 2),
-            (256, 5, 5, 4096, 1, 2), (256, 6, 8, 8, 0, 2), (128, 4, 1, 1, 0, 2), (0, 0, 0, 0, 0, 2)]:
+            (256, 5, 5, 4096, 1, 2), (256, 6, 8, 8, 0, 2), (128, 4, 1, 1, 0, 2), (0, 0, 0, 0, 0, 2),
+            (1024, 1, 0, 0, 0, 3), (1024, 1, 0, 0, 1, 4), (256, 2, 0, 0, 0, 4), (512, 1, 16, 0, 1, 3), (128, 4, 1, 4096, 0, 4),
+            (64, 3, 5, 4096, 1, 3), (256, 4, 8, 8, 0, 3), (32, 1, 0, 0, 0, 4), (0, 0, 0, 0, 0, 3), (0, 0, 0, 0, 1, 4)]:
         mode = (threads, per_sm, shared, total, order, family)
         lf.fire_set_launch_geometry(L, threads, per_sm)
         lf.fire_set_list_capacity(L, shared, total)
@@ -496,7 +498,7 @@ def test_genetic_algorithm_drives_the_batch_api(request):
 # ---------------------------------------------------------------------------------- randomised parity
 def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
     """Seeded fuzz: random lattice sizes (1 x 1 .. 140 x 200, ragged), vegetation, parameters, ignitions (some off the lattice
-    or on non-burnable cells), step limits, CTA sizes, residencies, list capacities, launch orders and both kernel families.
+    or on non-burnable cells), step limits, CTA sizes, residencies, list capacities, launch orders, both kernel families and cluster sizes.
     The oracle is fed the GPU's own threshold tables, so burned maps, steps and trial counts must be bit-exact."""
     rng = np.random.default_rng(20260604)
     n = 0
@@ -515,7 +517,7 @@ def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
         max_steps = int(rng.choice([0, 0, 0, 3, 17]))
         geom = (int(rng.choice([32, 64, 96, 128, 256, 512, 1024])), int(rng.integers(1, 9)))
         caps = (int(rng.choice([0, 0, 1, 4, 16])), int(rng.choice([0, 0, 0, 2, 64])))
-        order, family = int(rng.integers(0, 2)), int(rng.choice([0, 1, 2]))
+        order, family = int(rng.integers(0, 2)), int(rng.choice([0, 1, 2, 3, 4]))
         mode = (order, family)
         Lo = orc_landscape(orc, ls)
         L = gh.make_landscape(ls)
