@@ -75,30 +75,130 @@ fire_covariates_kernel(const uint8_t* __restrict__ veg, const float* __restrict_
 #define FIRE_THR_PGROUP 8
 constexpr int kThrTX = 32, kThrTY = 8;
 
-__device__ __forceinline__ uint32_t fire_threshold_from_x(double x)
+// T = min(rint(2^32 / (1 + exp(-x))), 2^32 - 1) in double precision, written for the FP64 pipe: the kernel is bound by it (about 30
+// double-precision operations per logistic with the library's exp and a correctly rounded reciprocal, 2.1e9 logistics per
+// generation), so every step is the cheapest one that keeps the result within a few ulp of p, i.e. within ONE count and only
+// when p 2^32 lies within 1e-6 of a rounding boundary (tests count these on the whole table of config 3; north_star allows <= 1):
+//   exp(y), |y| <= 40 (beyond |x| = 40 the threshold is saturated either way: p 2^32 rounds to 2^32 from x = 22.9 on and to 0
+//            below -22.9): y = (64 k + j) ln 2 / 64 + r with a Cody-Waite split of ln 2 / 64, 2^(j/64) from a 64-entry table in
+//            shared memory, exp(r) by a Taylor polynomial of degree 5 on |r| <= ln 2 / 128 (truncation 3e-17), 2^k added to the
+//            exponent field: 10 operations instead of 16;
+//   1 / d:   the hardware's 20-bit estimate and two Newton steps (full double precision, not correctly rounded);
+//   rint:    p 2^32 + 2^52 in ONE fused operation: the product is exact and the addition rounds it to an integer, ties to even
+//            (R-11), exactly as llrint(ldexp(p, 32)) does.
+__constant__ double kExp2Table[64] = {      // 2^(j/64), j = 0..63, correctly rounded
+    1.0, 1.0108892860517005, 1.0218971486541166, 1.0330248790212284,
+    1.0442737824274138, 1.0556451783605572, 1.0671404006768237, 1.0787607977571199,
+    1.0905077326652577, 1.102382583307841, 1.1143867425958924, 1.1265216186082418,
+    1.1387886347566916, 1.1511892299529827, 1.1637248587775775, 1.1763969916502812,
+    1.189207115002721, 1.202156731452703, 1.215247359980469, 1.22848053610687,
+    1.241857812073484, 1.255380757024691, 1.2690509571917332, 1.2828700160787783,
+    1.2968395546510096, 1.3109612115247644, 1.3252366431597413, 1.339667524053303,
+    1.3542555469368927, 1.3690024229745905, 1.383909881963832, 1.3989796725383112,
+    1.4142135623730951, 1.42961333839197, 1.4451808069770467, 1.460917794180647,
+    1.4768261459394993, 1.4929077282912648, 1.5091644275934228, 1.5255981507445384,
+    1.5422108254079407, 1.559004400237837, 1.5759808451078865, 1.593142151342267,
+    1.6104903319492543, 1.6280274218573478, 1.645755478153965, 1.6636765803267364,
+    1.681792830507429, 1.7001063537185235, 1.718619298122478, 1.7373338352737062,
+    1.7562521603732995, 1.7753764925265212, 1.7947090750031072, 1.8142521755003989,
+    1.8340080864093424, 1.8539791250833855, 1.8741676341103, 1.8945759815869656,
+    1.9152065613971474, 1.9360617934922943, 1.9571441241754002, 1.978456026387951
+};
+
+__device__ __forceinline__ uint32_t fire_threshold_from_x(double x, const double* __restrict__ tbl)
 {
-    const double e = exp(-x);
-    const double p = __drcp_rn(__dadd_rn(1.0, e));                        // Eq. 1: 1 / (1 + exp(-x)), correctly rounded reciprocal
-    const unsigned long long t = (unsigned long long)__double2ll_rn(p * 4294967296.0);   // exact scaling, ties-to-even (R-11); 0 <= t <= 2^32
-    return (uint32_t)t - (uint32_t)(t >> 32);                             // min(t, 2^32 - 1)
+    // clamp to [-40, 40] with integer operations on the high word (the FP64 pipe is the bottleneck)
+    double y = -x;
+    const uint32_t yh = (uint32_t)__double2hiint(y);
+    if ((yh & 0x7FFFFFFFu) >= 0x40440000u) y = __hiloint2double((int)((yh & 0x80000000u) | 0x40440000u), 0);
+    const double t = __fma_rn(y, 92.33248261689366, 6755399441055744.0);        // 2^52 + 2^51: low word = n = rint(64 y log2 e)
+    const double nf = t - 6755399441055744.0;
+    double r = __fma_rn(nf, -0.010830424667801708, y);                            // ln 2 / 64, high part (24 trailing zero bits)
+    r = __fma_rn(nf, -2.8447437476627285e-11, r);                                 // low part
+    double q = 8.33333333333333333333e-03;                                        // 1/120
+    q = __fma_rn(q, r, 4.16666666666666666667e-02);
+    q = __fma_rn(q, r, 1.66666666666666666667e-01);
+    q = __fma_rn(q, r, 0.5);
+    q = __fma_rn(q, r, 1.0);
+    q = __fma_rn(q, r, 1.0);
+    const int n = __double2loint(t);
+    q = q * tbl[n & 63];
+    const double e = __hiloint2double(__double2hiint(q) + ((n >> 6) << 20), __double2loint(q));   // q 2^k, |k| <= 58
+    const double d = 1.0 + e;
+    double rc;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(d));
+    rc = __fma_rn(rc, __fma_rn(-d, rc, 1.0), rc);
+    rc = __fma_rn(rc, __fma_rn(-d, rc, 1.0), rc);
+    const double v = __fma_rn(rc, 4294967296.0, 4503599627370496.0);              // 2^52 + rint(p 2^32), 0 <= rint <= 2^32
+    const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
+    return (hi & 1u) ? 0xFFFFFFFFu : lo;                                          // min(., 2^32 - 1)
+}
+
+// The same for N independent arguments, written step by step across them so that the N dependent chains interleave in the
+// instruction stream (one chain alone waits for the latency of every operation).
+template <int N>
+__device__ __forceinline__ void fire_thresholds_from_x(const double (&x)[N], const double* __restrict__ tbl, uint32_t (&T)[N])
+{
+    double y[N], t[N], r[N], q[N], d[N], rc[N];
+    int n[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        y[i] = -x[i];
+        const uint32_t yh = (uint32_t)__double2hiint(y[i]);
+        if ((yh & 0x7FFFFFFFu) >= 0x40440000u) y[i] = __hiloint2double((int)((yh & 0x80000000u) | 0x40440000u), 0);
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) t[i] = __fma_rn(y[i], 92.33248261689366, 6755399441055744.0);
+#pragma unroll
+    for (int i = 0; i < N; ++i) { const double nf = t[i] - 6755399441055744.0; r[i] = __fma_rn(nf, -0.010830424667801708, y[i]); r[i] = __fma_rn(nf, -2.8447437476627285e-11, r[i]); n[i] = __double2loint(t[i]); }
+#pragma unroll
+    for (int i = 0; i < N; ++i) q[i] = __fma_rn(8.33333333333333333333e-03, r[i], 4.16666666666666666667e-02);
+#pragma unroll
+    for (int i = 0; i < N; ++i) q[i] = __fma_rn(q[i], r[i], 1.66666666666666666667e-01);
+#pragma unroll
+    for (int i = 0; i < N; ++i) q[i] = __fma_rn(q[i], r[i], 0.5);
+#pragma unroll
+    for (int i = 0; i < N; ++i) q[i] = __fma_rn(q[i], r[i], 1.0);
+#pragma unroll
+    for (int i = 0; i < N; ++i) q[i] = __fma_rn(q[i], r[i], 1.0);
+#pragma unroll
+    for (int i = 0; i < N; ++i) q[i] = q[i] * tbl[n[i] & 63];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const double e = __hiloint2double(__double2hiint(q[i]) + ((n[i] >> 6) << 20), __double2loint(q[i]));
+        d[i] = 1.0 + e;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc[i]) : "d"(d[i]));
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) rc[i] = __fma_rn(rc[i], __fma_rn(-d[i], rc[i], 1.0), rc[i]);
+#pragma unroll
+    for (int i = 0; i < N; ++i) rc[i] = __fma_rn(rc[i], __fma_rn(-d[i], rc[i], 1.0), rc[i]);
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const double v = __fma_rn(rc[i], 4294967296.0, 4503599627370496.0);
+        const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
+        T[i] = (hi & 1u) ? 0xFFFFFFFFu : lo;
+    }
 }
 
 // x of Eq. 1 for one (target, direction): every operation one IEEE double operation, in the order of C-3
 __device__ __forceinline__ uint32_t fire_threshold(double b0, double b1, double b2, double b3, double b4,
-                                                   double If, double ps, double om, double sg)
+                                                   double If, double ps, double om, double sg, const double* __restrict__ tbl)
 {
     const double base = __dadd_rn(__dadd_rn(b0, __dmul_rn(b1, If)), __dmul_rn(b2, ps));
     const double x = __dadd_rn(__dadd_rn(base, __dmul_rn(b3, om)), __dmul_rn(b4, sg));
-    return fire_threshold_from_x(x);
+    return fire_threshold_from_x(x, tbl);
 }
 
-__global__ void __launch_bounds__(kThrTX * kThrTY)
+constexpr int kThrChains = 4;      // directions evaluated side by side (4 x 2 passes; 8 at once needs 108 registers and is slower)
+__global__ void __launch_bounds__(kThrTX * kThrTY, 4)
 fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int tiles_x,
                        const uint8_t* __restrict__ flags, const uint8_t* __restrict__ uphill,
                        const double* __restrict__ psi, const double* __restrict__ tan_slope,
                        const double* __restrict__ omega, uint32_t* __restrict__ thr, float* __restrict__ param_mean)
 {
     __shared__ double sb[FIRE_THR_PGROUP][5];
+    __shared__ double s_exp2[64];
     __shared__ float s_mean[FIRE_THR_PGROUP];
     __shared__ uint32_t sT2[2][8][kThrTY + 2][kThrTX + 2];                // [buffer][d][source row + 1][source column + 1]
     const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
@@ -106,6 +206,7 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
     const int np = min(FIRE_THR_PGROUP, P - p0);
     if (tid < np * 5) sb[tid / 5][tid % 5] = (double)beta[(size_t)p0 * 5 + tid];
     if (tid < FIRE_THR_PGROUP) s_mean[tid] = 0.0f;
+    if (tid < 64) s_exp2[tid] = kExp2Table[tid];
     const int x0 = (int)(blockIdx.x % tiles_x) * kThrTX, y0 = (int)(blockIdx.x / tiles_x) * kThrTY;
     const int x = x0 + lx, y = y0 + ly;
     const size_t cells = (size_t)W * H;
@@ -133,12 +234,26 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
         const double b0 = sb[q][0], b1 = sb[q][1], b2 = sb[q][2], b3 = sb[q][3], b4 = sb[q][4];
         uint32_t (*sT)[kThrTY + 2][kThrTX + 2] = sT2[q & 1];         // double-buffered: one barrier per parameter vector
         float fsum = 0.0f;
+        // Eq. 1 for the 8 directions of this target: x in the order of C-3, one IEEE operation each; non-burnable targets run
+        // the same arithmetic on zeros and are masked at the end (no branch: the chains of 4 directions interleave)
+        const double base = __dadd_rn(__dadd_rn(b0, __dmul_rn(b1, If)), __dmul_rn(b2, ps));
 #pragma unroll
-        for (int d = 0; d < 8; ++d) {
-            uint32_t T = 0u;
-            if (live) T = fire_threshold(b0, b1, b2, b3, b4, If, ps, om[d], ((up >> d) & 1u) ? ts : 0.0);
-            sT[d][ly - fire_dy(d) + 1][lx - fire_dx(d) + 1] = T;          // slot d of the source = target - offset(d)
-            fsum += (float)T * 2.3283064365386963e-10f;
+        for (int h = 0; h < 8 / kThrChains; ++h) {
+            double x4[kThrChains];
+            uint32_t T4[kThrChains];
+#pragma unroll
+            for (int i = 0; i < kThrChains; ++i) {
+                const int d = kThrChains * h + i;
+                x4[i] = __dadd_rn(__dadd_rn(base, __dmul_rn(b3, om[d])), __dmul_rn(b4, ((up >> d) & 1u) ? ts : 0.0));
+            }
+            fire_thresholds_from_x<kThrChains>(x4, s_exp2, T4);
+#pragma unroll
+            for (int i = 0; i < kThrChains; ++i) {
+                const int d = kThrChains * h + i;
+                const uint32_t T = live ? T4[i] : 0u;
+                sT[d][ly - fire_dy(d) + 1][lx - fire_dx(d) + 1] = T;      // slot d of the source = target - offset(d)
+                fsum += (float)T * 2.3283064365386963e-10f;
+            }
         }
         // scheduling hint only (never enters a result): sum of the contagion probabilities of this parameter vector
 #pragma unroll
@@ -198,7 +313,7 @@ fire_thresholds_gather_kernel(const float* __restrict__ beta5, int W, int H,
         T = 0u;
         if (f & 1u)
             T = fire_threshold((double)beta5[0], (double)beta5[1], (double)beta5[2], (double)beta5[3], (double)beta5[4],
-                               (f & 2u) ? 1.0 : 0.0, psi[c], omega[(size_t)d * cells + c], ((uphill[c] >> d) & 1u) ? tan_slope[c] : 0.0);
+                               (f & 2u) ? 1.0 : 0.0, psi[c], omega[(size_t)d * cells + c], ((uphill[c] >> d) & 1u) ? tan_slope[c] : 0.0, kExp2Table);
     }
     out[i] = T;
 }
