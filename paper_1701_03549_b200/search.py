@@ -95,19 +95,98 @@ class Evaluator:
         return score.cpu().numpy().astype(np.float64).reshape(P, R).mean(axis=1)
 
 
+@dataclass
+class IgnitionEvaluator:
+    """The 7-parameter case: an individual is (beta_0 .. beta_4, x, y) and starts its fires
+    from its own ignition cell (x, y rounded to the nearest cell and clipped to the lattice).  A cell that cannot burn burns
+    nothing (R-12), so Eq. 2 gives that individual delta = 1.  Scores of the last call stay on the device in `last_counts`
+    (u32 [P * replicates][2]) for fire_fitness_group_stats (a8: per-candidate mean and variance)."""
+    L: object
+    reference: object
+    replicates: int = 4
+    metric: int = 0
+    seed: int = 1
+    calls: int = field(default=0, init=False)
+    last_counts: object = field(default=None, init=False)
+
+    def cells_of(self, pop: np.ndarray) -> np.ndarray:
+        xy = np.rint(np.asarray(pop, np.float64)[:, 5:7]).astype(np.int64)
+        xy[:, 0] = np.clip(xy[:, 0], 0, self.L.W - 1)
+        xy[:, 1] = np.clip(xy[:, 1], 0, self.L.H - 1)
+        return xy.astype(np.int32)
+
+    def __call__(self, pop: np.ndarray) -> np.ndarray:
+        import torch
+        from . import libfire as lf
+        pop = np.asarray(pop, np.float64)
+        P, R = pop.shape[0], self.replicates
+        S = P * R
+        dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        lf.fire_params_upload(self.L, dev(pop[:, :5].astype(np.float32)))
+        ign = np.repeat(self.cells_of(pop), R, axis=0)
+        par = np.repeat(np.arange(P, dtype=np.int32), R)
+        seeds = (np.uint64(self.seed) << np.uint64(40)) | (np.uint64(self.calls) << np.uint64(20)) | np.arange(S, dtype=np.uint64)
+        burned = torch.empty((S, self.L.H, self.L.Ww), dtype=torch.int32, device="cuda")
+        lf.fire_simulate_batch(self.L, dev(ign), dev(par), dev(seeds.view(np.int64)), burned)
+        score = torch.empty((S,), dtype=torch.float32, device="cuda")
+        counts = torch.empty((S, 2), dtype=torch.int32, device="cuda")
+        lf.fire_fitness(self.L, self.reference, burned, self.metric, score, counts)
+        self.last_counts = counts
+        self.calls += 1
+        return score.cpu().numpy().astype(np.float64).reshape(P, R).mean(axis=1)
+
+
+def scar_cells(reference_bitmap: np.ndarray, W: int) -> np.ndarray:
+    """(x, y) of every burnt cell of a bit-packed map u32[H][ceil(W/32)]: the candidates the paper draws ignition points from
+    ("a random ignition point within the reference fire burnt area", PAPER.md:97)."""
+    words = np.ascontiguousarray(reference_bitmap, dtype="<u4")
+    bits = np.unpackbits(words.view(np.uint8), axis=-1, bitorder="little")[:, :W]
+    ys, xs = np.nonzero(bits)
+    return np.stack([xs, ys], 1).astype(np.int64)
+
+
+def initial_population_with_ignition(rng: np.random.Generator, lo, hi, scar: np.ndarray, pop_size: int) -> np.ndarray:
+    """Genes 0-4 uniform in [lo, hi]; genes 5-6 = a cell of the reference scar chosen at random."""
+    lo, hi = np.asarray(lo, np.float64), np.asarray(hi, np.float64)
+    pop = np.empty((pop_size, 7), np.float64)
+    pop[:, :5] = lo[:5] + rng.random((pop_size, 5)) * (hi[:5] - lo[:5])
+    pop[:, 5:7] = scar[rng.integers(0, scar.shape[0], pop_size)]
+    return pop
+
+
+def ensemble_estimate(individuals: np.ndarray, fitness: np.ndarray, cutoff: float):
+    """The paper's reading of a finished search (Tables 2-3): the best individual is the one of minimum fitness; the
+    estimate of every parameter is the mean, and its error the standard deviation, over the ensemble of simulated individuals
+    whose fitness is below `cutoff`.  Returns (best, mean, sd, ensemble size)."""
+    individuals, fitness = np.asarray(individuals, np.float64), np.asarray(fitness, np.float64)
+    ok = np.isfinite(fitness)
+    best = individuals[int(np.argmin(np.where(ok, fitness, np.inf)))].copy()
+    sel = ok & (fitness < cutoff)
+    if not sel.any():
+        return best, np.full(individuals.shape[1], np.nan), np.full(individuals.shape[1], np.nan), 0
+    ens = individuals[sel]
+    return best, ens.mean(axis=0), ens.std(axis=0, ddof=1) if ens.shape[0] > 1 else np.zeros(individuals.shape[1]), int(sel.sum())
+
+
 # ------------------------------------------------------------------------------------------ search loops
 def genetic_algorithm(evaluate, lo, hi, pop_size: int = 64, generations: int = 20, n_elite: int = 2,
-                      seed: int = 0, p_start: float = 0.25, p_end: float = 0.02):
-    """GA of PAPER.md App. B over the box [lo, hi].  `evaluate(pop) -> fitness` (lower is better).
+                      seed: int = 0, p_start: float = 0.25, p_end: float = 0.02, init: np.ndarray | None = None,
+                      archive: list | None = None):
+    """GA of PAPER.md App. B over the box [lo, hi].  `evaluate(pop) -> fitness` (lower is better).  `init`: first population
+    (default: uniform in the box).  `archive`: if a list, every evaluated (population, fitness) pair is appended to it (the
+    ensemble the paper's histograms and error bars are made of).
     Returns (best vector, best fitness, history of (generation, best, mean))."""
     rng = np.random.Generator(np.random.PCG64(seed))
     lo, hi = np.asarray(lo, np.float64), np.asarray(hi, np.float64)
-    pop = lo + rng.random((pop_size, lo.shape[0])) * (hi - lo)
+    pop = lo + rng.random((pop_size, lo.shape[0])) * (hi - lo) if init is None else np.clip(np.asarray(init, np.float64), lo, hi)
+    pop_size = pop.shape[0]
     history = []
     best_vec, best_fit = None, np.inf
     for gen in range(generations):
         fit = np.asarray(evaluate(pop), np.float64)
         fit = np.where(np.isfinite(fit), fit, np.inf)
+        if archive is not None:
+            archive.append((pop.copy(), fit.copy()))
         k = int(np.argmin(fit))
         if fit[k] < best_fit:
             best_vec, best_fit = pop[k].copy(), float(fit[k])

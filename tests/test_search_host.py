@@ -55,3 +55,35 @@ def test_ga_and_monte_carlo_minimise_a_known_function():
     assert all(b2 <= b1 + 1e-12 for b1, b2 in zip(bests, bests[1:]))       # elitism: the best never gets worse on a deterministic function
     samples, fits = search.monte_carlo(f, lo, hi, n_samples=4096, batch=500, seed=4)
     assert (np.diff(fits) >= 0).all() and fits[0] < 1.0 and samples.shape == (4096, 5)
+
+
+def test_scar_cells_initial_population_and_ensemble_estimate():
+    """SURVEY 8 f2 host pieces: candidates come from the reference scar, the estimate and its error from the
+    ensemble below a fitness cutoff."""
+    mask = np.zeros((5, 40), bool)
+    mask[1, 3] = mask[4, 33] = mask[2, 31] = mask[2, 32] = True
+    Ww = 2
+    words = np.zeros((5, Ww), np.uint32)
+    for y, x in zip(*np.nonzero(mask)):
+        words[y, x >> 5] |= np.uint32(1) << np.uint32(x & 31)
+    cells = search.scar_cells(words, 40)
+    assert sorted(map(tuple, cells.tolist())) == sorted([(3, 1), (33, 4), (31, 2), (32, 2)])
+    rng = np.random.default_rng(0)
+    lo, hi = np.array([-1.0, -2, -3, -4, -5, 0, 0]), np.array([1.0, 2, 3, 4, 5, 39, 4])
+    pop = search.initial_population_with_ignition(rng, lo, hi, cells, 500)
+    assert pop.shape == (500, 7) and (pop[:, :5] >= lo[:5]).all() and (pop[:, :5] <= hi[:5]).all()
+    assert set(map(tuple, pop[:, 5:7].astype(int).tolist())) == set(map(tuple, cells.tolist()))      # every candidate is a scar cell
+    ind = np.array([[0.0, 10], [1.0, 20], [2.0, 30], [3.0, 40]]); fit = np.array([0.5, 0.1, 0.2, np.inf])
+    best, mean, sd, n = search.ensemble_estimate(ind, fit, cutoff=0.3)
+    assert (best == [1.0, 20]).all() and n == 2 and np.allclose(mean, [1.5, 25]) and np.allclose(sd, np.std([[1.0, 20], [2.0, 30]], axis=0, ddof=1))
+    assert search.ensemble_estimate(ind, fit, cutoff=0.01)[3] == 0
+
+
+def test_ga_with_initial_population_and_archive():
+    target = np.array([0.3, -1.2])
+    f = lambda pop: ((np.asarray(pop) - target) ** 2).sum(axis=1)
+    init = np.full((32, 2), 2.5)
+    arch = []
+    best, fit, hist = search.genetic_algorithm(f, [-3, -3], [3, 3], generations=30, n_elite=2, seed=1, init=init, archive=arch)
+    assert len(arch) == 30 and arch[0][0].shape == (32, 2) and (arch[0][0] == 2.5).all()
+    assert fit < f(init[:1])[0]
