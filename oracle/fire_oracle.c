@@ -264,6 +264,103 @@ int orc_simulate(const uint8_t* veg, const float* slope, const float* aspect, co
     return 0;
 }
 
+/* ---------------------------------------------------------------------------
+ * C-4', fuel-dependent burn-out time (reading R-21).
+ * PAPER.md:91 "A burnt cell gets inactive after a given time that depends on the vegetation type of the cell", :145
+ * "cells have a turn off time that depends on vegetation fuel type", :68 / :273 (fuel consumption times are the extension the
+ * authors announce).  burn_time[v] >= 1 is that time, in steps, for vegetation class v (0 is read as 1).  A cell ignited by
+ * the transition t -> t+1 is ACTIVE during steps t+1 .. t+burn_time (the ignition cell during steps 0 .. burn_time-1); at
+ * every step every active cell is a source for each of its susceptible neighbours: one trial rnd(seed, sim, t, target, d)
+ * against T(target, d), exactly as in C-4 (the key contains the step, so a pair that is tried again draws a fresh word).
+ * The run ends when no cell is active.  burn_time == 1 everywhere is orc_simulate, byte for byte.
+ * out_time: optional, step at which the cell ignited (0 = ignition, -1 never).
+ * counters: trials, candidate cell-steps, distinct targets, as in orc_simulate.
+ * ------------------------------------------------------------------------- */
+int orc_simulate_burn_time(const uint8_t* veg, const float* slope, const float* aspect, const float* wind,
+                           int W, int H, const float beta[5], const uint32_t* table, const uint8_t burn_time[256],
+                           int ix, int iy, uint64_t seed, uint32_t sim, uint32_t max_steps,
+                           uint32_t* out_burned, int32_t* out_time, uint32_t* out_steps, uint64_t* counters)
+{
+    size_t ncell = (size_t)W * H;
+    int Ww = (W + 31) / 32;
+    uint8_t*  burned   = (uint8_t*)calloc(ncell, 1);
+    uint8_t*  is_new   = (uint8_t*)calloc(ncell, 1);
+    uint8_t*  left     = (uint8_t*)calloc(ncell, 1);    /* steps the cell stays active, 0 = inactive */
+    uint32_t* tried_at = (uint32_t*)calloc(ncell, 4);
+    uint32_t* active   = (uint32_t*)malloc(ncell * 4);  /* list of active cells */
+    uint32_t* next     = (uint32_t*)malloc(ncell * 4);
+    uint32_t* fresh    = (uint32_t*)malloc(ncell * 4);
+    if (!burned || !is_new || !left || !tried_at || !active || !next || !fresh) {
+        free(burned); free(is_new); free(left); free(tried_at); free(active); free(next); free(fresh);
+        return -1;
+    }
+    size_t n_active = 0;
+    uint64_t trials = 0, cand_steps = 0, distinct = 0;
+    uint32_t t = 0;
+    if (out_time) for (size_t c = 0; c < ncell; ++c) out_time[c] = -1;
+
+    if (ix >= 0 && ix < W && iy >= 0 && iy < H && veg[(size_t)iy * W + ix] != 0) {
+        size_t c = (size_t)iy * W + ix;
+        burned[c] = 1;
+        left[c] = burn_time[veg[c]] ? burn_time[veg[c]] : 1;
+        active[n_active++] = (uint32_t)c;
+        if (out_time) out_time[c] = 0;
+    }
+
+    while (n_active > 0 && (max_steps == 0 || t < max_steps)) {
+        size_t n_fresh = 0, n_next = 0;
+        for (size_t i = 0; i < n_active; ++i) {
+            int sx = (int)(active[i] % (uint32_t)W), sy = (int)(active[i] / (uint32_t)W);
+            for (int d = 0; d < 8; ++d) {
+                int tx = sx + DX[d], ty = sy + DY[d];
+                if (tx < 0 || tx >= W || ty < 0 || ty >= H) continue;
+                size_t c = (size_t)ty * W + tx;
+                if (veg[c] == 0) continue;
+                if (burned[c]) continue;
+                ++trials;
+                if (tried_at[c] != t + 1) {
+                    if (tried_at[c] == 0) ++distinct;
+                    tried_at[c] = t + 1;
+                    ++cand_steps;
+                }
+                uint32_t T = table ? table[c * 8 + d]
+                                   : orc_threshold(beta, veg[c], slope[c], aspect[c], wind[c], d);
+                uint32_t r = orc_rnd(seed, sim, t, (uint32_t)c, d);
+                if (orc_trial_succeeds(r, T) && !is_new[c]) {
+                    is_new[c] = 1;
+                    fresh[n_fresh++] = (uint32_t)c;
+                }
+            }
+        }
+        /* synchronous update: one step of fuel is consumed in every active cell; the newly ignited become active */
+        for (size_t i = 0; i < n_active; ++i) {
+            size_t c = active[i];
+            if (--left[c] > 0) next[n_next++] = (uint32_t)c;
+        }
+        for (size_t i = 0; i < n_fresh; ++i) {
+            size_t c = fresh[i];
+            burned[c] = 1;
+            is_new[c] = 0;
+            left[c] = burn_time[veg[c]] ? burn_time[veg[c]] : 1;
+            next[n_next++] = (uint32_t)c;
+            if (out_time) out_time[c] = (int32_t)(t + 1);
+        }
+        uint32_t* tmp = active; active = next; next = tmp;
+        n_active = n_next;
+        ++t;
+    }
+
+    memset(out_burned, 0, (size_t)H * Ww * 4);
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x)
+            if (burned[(size_t)y * W + x])
+                out_burned[(size_t)y * Ww + (x >> 5)] |= (1u << (x & 31));
+    if (out_steps) *out_steps = t;
+    if (counters) { counters[0] = trials; counters[1] = cand_steps; counters[2] = distinct; }
+    free(burned); free(is_new); free(left); free(tried_at); free(active); free(next); free(fresh);
+    return 0;
+}
+
 /* A batch of independent simulations (each individual /
  * replicate is its own CA run).  Parallel over simulations only; each one is
  * orc_simulate unchanged.  tables: NULL, or P pointers (each NULL or u32[H][W][8]).

@@ -77,6 +77,10 @@ def _declare(l):
                                C.c_int, C.c_int, C.c_uint64, C.c_uint32, C.c_uint32,
                                _u32p, _i32p, _u32p, _u64p]
     l.orc_simulate.restype = C.c_int
+    l.orc_simulate_burn_time.argtypes = [_u8p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _f32p, _u32p, _u8p,
+                                         C.c_int, C.c_int, C.c_uint64, C.c_uint32, C.c_uint32,
+                                         _u32p, _i32p, _u32p, _u64p]
+    l.orc_simulate_burn_time.restype = C.c_int
     l.orc_simulate_batch.argtypes = [_u8p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _f32p, C.c_int,
                                      C.POINTER(_u32p), _i32p, _i32p, _u64p, _i32p, C.c_int,
                                      C.c_uint32, _u32p, _u32p, _u64p, C.c_int]
@@ -189,6 +193,30 @@ def simulate(L: Landscape, beta, ignition, seed: int, sim: int = 0, max_steps: i
                             C.byref(steps), _p(counters, _u64p))
     if rc != 0:
         raise MemoryError("orc_simulate failed")
+    return {"burned": burned, "steps": int(steps.value), "trials": int(counters[0]),
+            "cand_steps": int(counters[1]), "distinct": int(counters[2]), "time": time}
+
+
+def simulate_burn_time(L: Landscape, beta, burn_time, ignition, seed: int, sim: int = 0, max_steps: int = 0,
+                       table: np.ndarray | None = None, want_time: bool = False):
+    """One simulation with fuel-dependent burn-out times (C-4', R-21): burn_time[v] = steps a cell of class v stays active."""
+    b = _c(beta, np.float32)
+    bt = np.zeros(256, np.uint8)
+    bt[: len(burn_time)] = np.asarray(burn_time, np.uint8)
+    burned = np.zeros((L.H, L.Ww), np.uint32)
+    steps = C.c_uint32(0)
+    counters = np.zeros(3, np.uint64)
+    time = np.zeros((L.H, L.W), np.int32) if want_time else None
+    tab = None
+    if table is not None:
+        tab = _c(table, np.uint32)
+        assert tab.shape == (L.H, L.W, 8)
+    rc = lib().orc_simulate_burn_time(*L._ptrs(), L.W, L.H, _p(b, _f32p), _p(tab, _u32p) if tab is not None else None,
+                                      _p(bt, _u8p), int(ignition[0]), int(ignition[1]), int(seed), int(sim),
+                                      int(max_steps), _p(burned, _u32p), _p(time, _i32p) if want_time else None,
+                                      C.byref(steps), _p(counters, _u64p))
+    if rc != 0:
+        raise MemoryError("orc_simulate_burn_time failed")
     return {"burned": burned, "steps": int(steps.value), "trials": int(counters[0]),
             "cand_steps": int(counters[1]), "distinct": int(counters[2]), "time": time}
 
