@@ -91,6 +91,15 @@ int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, const int32
                         const uint64_t* seeds, const int32_t* sim_ids, int32_t S, uint32_t max_steps,
                         uint32_t* out_burned, uint32_t* out_steps, uint64_t* out_trials, void* stream);
 
+/* Fuel-dependent burn-out time ("a burnt cell gets inactive after a given time that depends on the
+ * vegetation type", :145, :68, :273; reading R-21).  burn_time_host u8[n_classes] (HOST memory, read before the call
+ * returns): steps a cell of vegetation class v stays ACTIVE once ignited, 1..8 (0 reads as 1; classes >= n_classes burn one
+ * step).  An active cell is a source for each of its susceptible neighbours at EVERY step it is active: one trial
+ * rnd(seed, sim, t, target, d) per step and pair, keyed as in fire_simulate_batch (the key holds the step, so a repeated pair
+ * draws a fresh word); the run ends when no cell is active.  All ones (or n_classes = 0) is the paper's setting and the default.
+ * Applies to every later fire_simulate_batch / fire_generation_host on this handle. */
+int fire_set_burn_time(fire_landscape* L, const uint8_t* burn_time_host, int32_t n_classes, void* stream);
+
 /* Fitness reduction (a7; Eq. 2).  reference u32[H][ceil(W/32)] = A, burned
  * u32[S][H][ceil(W/32)] = A*.  out_counts u32[S][2] or NULL = (I, N*) with I = #(A n A*), N* = #A*;
  * out_score f32[S]: metric 0 = (float)(N + N* - 2I) / (float)N, metric 1 = (float)I / (float)(N + N* - I),

@@ -49,6 +49,13 @@ struct fire_landscape {
     uint32_t* rescue_planes;      // rescue kernel: 2 burning planes per rescue CTA, kept all-zero between sims
     size_t    rescue_capacity;    // bytes
 
+    // f3: fuel-dependent burn-out times (fire_set_burn_time)
+    uint8_t*  veg_class;          // [cells] the caller's vegetation classes (kept: burn times are per class)
+    uint8_t*  ktime;              // [cells] burn time - 1 of the cell's class
+    uint32_t* gt_planes;          // [7][H][Ww] bit set iff burn time > j + 1
+    size_t    gt_capacity;
+    int       burn_kmax;          // largest burn time set; <= 1 = the base model (every cell burns one step)
+
     // a7: fitness scratch
     uint32_t* ref_area;           // [1]
     uint32_t* counts_scratch;     // [S][2] when the caller passes out_counts = NULL

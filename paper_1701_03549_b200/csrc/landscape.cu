@@ -329,7 +329,7 @@ extern "C" int fire_landscape_destroy(fire_landscape* L)
         cudaDeviceSynchronize();
         void* ptrs[] = { L->flags, L->uphill, L->psi, L->tan_slope, L->omega, L->burnable, L->thr, L->beta_dev,
                          L->work_counter, L->status, L->spill, L->rescue_planes, L->ref_area, L->counts_scratch,
-                         L->burnable_tiles, L->tiles, L->order, L->param_mean,
+                         L->burnable_tiles, L->tiles, L->order, L->param_mean, L->veg_class, L->ktime, L->gt_planes,
                          L->gen_buf };
         for (void* p : ptrs) if (p) cudaFree(p);
         if (L->prof_ev[0]) for (int i = 0; i < 2 * 64; ++i) if (L->prof_ev[i]) cudaEventDestroy(L->prof_ev[i]);
@@ -361,6 +361,7 @@ extern "C" int fire_landscape_create(fire_landscape** out, const uint8_t* veg, c
     bool ok = cudaMalloc(&L->flags, n) == cudaSuccess && cudaMalloc(&L->uphill, n) == cudaSuccess &&
               cudaMalloc(&L->psi, n * 8) == cudaSuccess && cudaMalloc(&L->tan_slope, n * 8) == cudaSuccess &&
               cudaMalloc(&L->omega, n * 64) == cudaSuccess && cudaMalloc(&L->burnable, nw * 4) == cudaSuccess &&
+              cudaMalloc(&L->veg_class, n) == cudaSuccess &&
               cudaMalloc(&L->work_counter, 4 * sizeof(unsigned int)) == cudaSuccess &&
               cudaMalloc(&L->ref_area, 4 * sizeof(uint32_t)) == cudaSuccess;
     if (!ok) { (void)cudaGetLastError(); fire_landscape_destroy(L); return FIRE_ENOMEM; }
@@ -368,6 +369,7 @@ extern "C" int fire_landscape_create(fire_landscape** out, const uint8_t* veg, c
     const long long threads = (long long)nw * 32;
     const int block = 256;
     const unsigned grid = (unsigned)((threads + block - 1) / block);
+    if (cudaMemcpyAsync(L->veg_class, veg, n, cudaMemcpyDeviceToDevice, st) != cudaSuccess) { (void)cudaGetLastError(); fire_landscape_destroy(L); return FIRE_ECUDA; }
     fire_covariates_kernel<<<grid, block, 0, st>>>(veg, slope, aspect, wind, W, H, L->Ww, L->flags, L->uphill, L->psi,
                                                    L->tan_slope, L->omega, L->burnable);
     L->launches += 1;

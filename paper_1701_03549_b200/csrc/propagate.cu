@@ -51,6 +51,9 @@ struct prop_params {
     uint32_t max_steps;
     uint32_t capA_s, capQ_s;      // shared-memory entries: each frontier list, the trial queue
     uint32_t capA, capQ;          // total entries (shared + spill); capQ >= 8 * capA
+    const uint8_t* ktime;         // [cells] burn time - 1 of the cell's fuel (fire_set_burn_time), or null
+    const uint32_t* gt_planes;    // [kmax - 1][H][Ww] bit set iff the cell's burn time > j + 1 (rescue kernel), or null
+    int kmax;                     // largest burn time (1 = every cell burns for one step)
 };
 
 __device__ __forceinline__ uint32_t lanemask_lt()
@@ -140,11 +143,30 @@ struct step_ctx {
     uint32_t cntQ, cntA_next, over;       // shared-window addresses of the queue counter, the next frontier's counter, the overflow flag
     uint32_t nA, nQ;
     uint32_t lane, lt;
+    const uint8_t* ktime;         // burn-time variant only
 };
+
+// Appends `entry` of the lanes with `flag` to the next frontier list (shared memory, then the global spill, then overflow).
+__device__ __forceinline__ void append_next(const step_ctx& c, bool flag, uint32_t entry)
+{
+    const uint32_t m = __ballot_sync(0xFFFFFFFFu, flag);
+    if (m == 0u) return;                                           // warp-uniform
+    uint32_t base = 0;
+    if (c.lane == 0) base = atoms_add(c.cntA_next, (uint32_t)__popc(m));
+    base = __shfl_sync(0xFFFFFFFFu, base, 0);
+    if (flag) {
+        const uint32_t pos = base + __popc(m & c.lt);
+        if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, entry);
+        else if (pos < c.capA) __stcg(c.spill + (c.an_off + (pos - c.capA_s)), entry);
+        else sts32(c.over, 1u);
+    }
+}
 
 // Phase 1 for K units of 32 burning cells (units u0, u0 + ustride, ...; all of them exist: u * 32 < nA).
 // Lanes past the end of the list re-read the last entry and contribute nothing.
-template <int K>
+// kBT (fuel-dependent burn-out time, R-21): bits 29..31 of a frontier entry = the steps the cell stays active AFTER this one;
+// a cell that has some left appends itself to the next frontier (it is a source again next step).
+template <int K, bool kBT = false>
 __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, uint32_t ustride)
 {
     uint32_t e[K], win[K];
@@ -157,7 +179,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         live[k] = i < c.nA;
         i = live[k] ? i : c.nA - 1u;
         e[k] = (i < c.capA_s) ? lds32(c.ac_addr + 4u * i) : __ldcg(c.spill + (c.ac_off + (i - c.capA_s)));
-        const uint32_t x = e[k] & 0xFFFFu, y = e[k] >> 16;
+        const uint32_t x = e[k] & 0xFFFFu, y = kBT ? ((e[k] >> 16) & 0x1FFFu) : (e[k] >> 16);
         const uint32_t tx0 = x >> 3, ty0 = y >> 3, bx = x & 7u, by = y & 7u;
         const uint32_t tidx = ty0 * c.Tw + tx0;
         const int hoff = (bx == 0u && tx0 > 0u) ? -1 : ((bx == 7u && tx0 + 1u < c.Tw) ? 1 : 0);
@@ -190,6 +212,13 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         const uint32_t hb = (bx == 0u) ? ((w3h >> 7) & 0x010101u) : ((w3h << 2) & 0x040404u);
         win[k] = live[k] ? ((tcen & mC) | hb) : 0u;
         cnt += __popc(win[k]);
+    }
+    if (kBT) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            append_next(c, live[k] && (e[k] >> 29) != 0u, e[k] - (1u << 29));      // still burning next step
+            e[k] &= 0x1FFFFFFFu;                                                   // the trial items are built from the coordinates
+        }
     }
     uint32_t incl = cnt;
 #pragma unroll
@@ -308,7 +337,7 @@ __device__ __forceinline__ void trials_issue(const step_ctx& c, const philox_ste
     }
 }
 
-template <int K>
+template <int K, bool kBT = false>
 __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_trials& pt)
 {
     uint32_t fresh_mask[K];
@@ -325,9 +354,12 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
     if (abase + n_fresh <= c.capA_s) {                             // warp-uniform: all new cells go to shared memory
 #pragma unroll
         for (int u = 0; u < K; ++u) {
-            const uint32_t en = pt.item[u] & 0xFFFF1FFFu;
+            uint32_t en = pt.item[u] & 0xFFFF1FFFu;
             const uint32_t a = c.an_addr + 4u * (abase + __popc(fresh_mask[u] & c.lt));
-            if (fresh_mask[u] & (1u << c.lane)) sts32(a, en);
+            if (fresh_mask[u] & (1u << c.lane)) {
+                if (kBT) en |= (uint32_t)__ldg(c.ktime + ((en >> 16) * c.W + (en & 0x1FFFu))) << 29;      // burn time of its fuel - 1
+                sts32(a, en);
+            }
             abase += __popc(fresh_mask[u]);
         }
     } else {
@@ -335,7 +367,8 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
         for (int u = 0; u < K; ++u) {
             if (fresh_mask[u] & (1u << c.lane)) {
                 const uint32_t pos = abase + __popc(fresh_mask[u] & c.lt);
-                const uint32_t en = pt.item[u] & 0xFFFF1FFFu;
+                uint32_t en = pt.item[u] & 0xFFFF1FFFu;
+                if (kBT) en |= (uint32_t)__ldg(c.ktime + ((en >> 16) * c.W + (en & 0x1FFFu))) << 29;
                 if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, en);
                 else if (pos < c.capA) __stcg(c.spill + (c.an_off + (pos - c.capA_s)), en);
                 else sts32(c.over, 1u);
@@ -356,13 +389,13 @@ __device__ __forceinline__ void trials_issue_k(const step_ctx& c, const philox_s
     else if (KMAX >= 2 && k == 2) trials_issue<2>(c, ph, u0, ustride, pt);
     else trials_issue<1>(c, ph, u0, ustride, pt);
 }
-template <int KMAX>
+template <int KMAX, bool kBT = false>
 __device__ __forceinline__ void trials_resolve_k(const step_ctx& c, int k, const pending_trials& pt)
 {
-    if (KMAX >= 4 && k == 4) trials_resolve<4>(c, pt);
-    else if (KMAX >= 3 && k == 3) trials_resolve<3>(c, pt);
-    else if (KMAX >= 2 && k == 2) trials_resolve<2>(c, pt);
-    else if (k == 1) trials_resolve<1>(c, pt);
+    if (KMAX >= 4 && k == 4) trials_resolve<4, kBT>(c, pt);
+    else if (KMAX >= 3 && k == 3) trials_resolve<3, kBT>(c, pt);
+    else if (KMAX >= 2 && k == 2) trials_resolve<2, kBT>(c, pt);
+    else if (k == 1) trials_resolve<1, kBT>(c, pt);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -370,7 +403,7 @@ __device__ __forceinline__ void trials_resolve_k(const step_ctx& c, int k, const
 // Instantiated for a few (threads per CTA, CTAs per SM) bounds: the bound sets the register budget.
 // kCellsInFlight / kTrialsInFlight: units of 32 burning cells (phase 1) / 32 trials (phase 2) a warp has in flight.
 // ------------------------------------------------------------------------------------------------
-template <int kMaxThreads, int kMinCtas, int kCellsInFlight, int kTrialsInFlight>
+template <int kMaxThreads, int kMinCtas, int kCellsInFlight, int kTrialsInFlight, bool kBT = false>
 __global__ void __launch_bounds__(kMaxThreads, kMinCtas)
 fire_propagate_kernel(const prop_params prm)
 {
@@ -403,6 +436,7 @@ fire_propagate_kernel(const prop_params prm)
     const uint32_t cntQ_addr = cntA_addr + 8u;
     c.over = cntA_addr + 16u;
     c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
+    c.ktime = prm.ktime;
 
     for (;;) {
         __syncthreads();                       // the previous simulation's last reads of s_* are done
@@ -431,7 +465,8 @@ fire_propagate_kernel(const prop_params prm)
             s_cntA[0] = valid ? 1u : 0u; s_cntA[1] = 0u; s_cntQ[0] = 0u; s_cntQ[1] = 0u;
             s_over = 0u; s_trials = 0ull;
             if (valid) {
-                const uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
+                uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
+                if (kBT) e0 |= (uint32_t)prm.ktime[(size_t)iy * prm.W + ix] << 29;
                 if (prm.capA_s > 0) sts32(as_addr0, e0); else prm.spill[ag_off0] = e0;
                 atomicAnd(reinterpret_cast<uint32_t*>(prm.tiles) + (((size_t)c.plane_w + (size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
@@ -453,8 +488,8 @@ fire_propagate_kernel(const prop_params prm)
                 const uint32_t nU = (c.nA + 31u) >> 5;
                 uint32_t u = warp;
                 for (; u + (uint32_t)(kCellsInFlight - 1) * nwarps < nU; u += nwarps * kCellsInFlight)
-                    my_trials += cells_pass<kCellsInFlight>(c, u, nwarps);
-                for (; u < nU; u += nwarps) my_trials += cells_pass<1>(c, u, nwarps);
+                    my_trials += cells_pass<kCellsInFlight, kBT>(c, u, nwarps);
+                for (; u < nU; u += nwarps) my_trials += cells_pass<1, kBT>(c, u, nwarps);
             }
             __syncthreads();
             c.nQ = s_cntQ[par];
@@ -485,16 +520,16 @@ fire_propagate_kernel(const prop_params prm)
                     for (; left >= (uint32_t)kTrialsInFlight; left -= (uint32_t)kTrialsInFlight, u += nwarps * kTrialsInFlight) {
                         pending_trials cur;
                         trials_issue<kTrialsInFlight>(c, ph, u, nwarps, cur);
-                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
+                        if (have) trials_resolve<kTrialsInFlight, kBT>(c, prev);
                         prev = cur; have = true;
                     }
                     if (left > 0u) {                               // the last, shorter pass: specialised by its exact size
                         pending_trials cur;
                         trials_issue_k<kTrialsInFlight>(c, ph, u, nwarps, (int)left, cur);
-                        if (have) trials_resolve<kTrialsInFlight>(c, prev);
-                        trials_resolve_k<kTrialsInFlight>(c, (int)left, cur);
+                        if (have) trials_resolve<kTrialsInFlight, kBT>(c, prev);
+                        trials_resolve_k<kTrialsInFlight, kBT>(c, (int)left, cur);
                     } else if (have) {
-                        trials_resolve<kTrialsInFlight>(c, prev);
+                        trials_resolve<kTrialsInFlight, kBT>(c, prev);
                     }
                 }
             }
@@ -1028,6 +1063,149 @@ fire_propagate_rescue_kernel(const prop_params prm, uint32_t* planes)
     }
 }
 
+// The rescue kernel for fuel-dependent burn-out times (R-21).  planes: [gridDim.x][kmax + 1][H*Ww], a ring of "ignited by the
+// transition into state tau" planes, all-zero on entry and on exit; a cell is active at step t iff it ignited at tau = t - j with
+// burn time > j, i.e. active(t) = OR_j ring[(t - j) mod (kmax + 1)] & gt[j] with gt[0] = everything, gt[j] = prm.gt_planes[j - 1].
+__device__ __forceinline__ uint32_t active_word(const prop_params& prm, const uint32_t* ring, size_t nw, uint32_t t, int y, int wx)
+{
+    if ((unsigned)y >= (unsigned)prm.H || (unsigned)wx >= (unsigned)prm.Ww) return 0u;
+    const size_t wi = (size_t)y * prm.Ww + wx;
+    const uint32_t R1 = (uint32_t)prm.kmax + 1u;
+    uint32_t a = __ldcg(ring + (size_t)(t % R1) * nw + wi);
+    for (uint32_t j = 1; j < (uint32_t)prm.kmax && j <= t; ++j)
+        a |= __ldcg(ring + (size_t)((t - j) % R1) * nw + wi) & __ldg(prm.gt_planes + (size_t)(j - 1) * nw + wi);
+    return a;
+}
+
+__global__ void __launch_bounds__(256)
+fire_propagate_rescue_bt_kernel(const prop_params prm, uint32_t* planes)
+{
+    __shared__ int s_y0, s_y1;
+    __shared__ unsigned long long s_trials;
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int W = prm.W, H = prm.H, Ww = prm.Ww;
+    const size_t nw = (size_t)H * Ww;
+    const uint32_t R1 = (uint32_t)prm.kmax + 1u;
+    const unsigned int n_rescue = *((volatile unsigned int*)(prm.work_counter + 1));
+
+    for (unsigned int k = blockIdx.x; k < n_rescue; k += gridDim.x) {
+        const uint32_t s = prm.rescue_list[k];
+        const int p = prm.sim_param[s];
+        const int ix = prm.ignitions[2 * s], iy = prm.ignitions[2 * s + 1];
+        const uint64_t seed = prm.seeds[s];
+        const uint32_t key_lo = (uint32_t)seed, key_hi = (uint32_t)(seed >> 32);
+        const uint32_t sim = prm.sim_ids ? (uint32_t)prm.sim_ids[s] : s;
+        const uint32_t* const thr = prm.thr + (size_t)p * W * H * 8;
+        uint32_t* const burned = prm.out_burned + (size_t)s * nw;
+        uint32_t* const ring = planes + (size_t)blockIdx.x * R1 * nw;
+
+        for (size_t w = tid; w < nw; w += nthr) burned[w] = 0u;      // the fast kernel left it half-done
+        if (tid == 0) { s_y0 = iy; s_y1 = iy; s_trials = 0ull; }
+        __syncthreads();
+        if (tid == 0) {
+            burned[(size_t)iy * Ww + (ix >> 5)] = 1u << (ix & 31);
+            ring[(size_t)iy * Ww + (ix >> 5)] = 1u << (ix & 31);      // ignited "by the transition into state 0"
+        }
+        __syncthreads();
+
+        uint32_t t = 0;
+        unsigned long long my_trials = 0;
+        int burning = 1;
+        while (burning && (prm.max_steps == 0 || t < prm.max_steps)) {
+            const int ylo = max(s_y0 - 1, 0), yhi = min(s_y1 + 1, H - 1);
+            const int nwords = (yhi - ylo + 1) * Ww;
+            uint32_t* const nxt = ring + (size_t)((t + 1u) % R1) * nw;
+            int any_new = 0, ny0 = H, ny1 = -1;
+            for (int idx = tid; idx < nwords; idx += nthr) {
+                const int y = ylo + idx / Ww, wx = idx % Ww;
+                const uint32_t uL = active_word(prm, ring, nw, t, y - 1, wx - 1), uC = active_word(prm, ring, nw, t, y - 1, wx),
+                               uR = active_word(prm, ring, nw, t, y - 1, wx + 1);
+                const uint32_t mL = active_word(prm, ring, nw, t, y, wx - 1), mC = active_word(prm, ring, nw, t, y, wx),
+                               mR = active_word(prm, ring, nw, t, y, wx + 1);
+                const uint32_t dL = active_word(prm, ring, nw, t, y + 1, wx - 1), dC = active_word(prm, ring, nw, t, y + 1, wx),
+                               dR = active_word(prm, ring, nw, t, y + 1, wx + 1);
+                uint32_t src[8];
+                src[0] = dC;
+                src[1] = (dC << 1) | (dL >> 31);
+                src[2] = (mC << 1) | (mL >> 31);
+                src[3] = (uC << 1) | (uL >> 31);
+                src[4] = uC;
+                src[5] = (uC >> 1) | (uR << 31);
+                src[6] = (mC >> 1) | (mR << 31);
+                src[7] = (dC >> 1) | (dR << 31);
+                const size_t wi = (size_t)y * Ww + wx;
+                const uint32_t sus = __ldg(prm.burnable + wi) & ~__ldcg(burned + wi);
+                uint32_t cand = (src[0] | src[1] | src[2] | src[3] | src[4] | src[5] | src[6] | src[7]) & sus;
+                uint32_t fresh = 0;
+                while (cand) {
+                    const int bx = __ffs(cand) - 1;
+                    cand &= cand - 1;
+                    const uint32_t c = (uint32_t)(y * W + wx * 32 + bx);
+                    bool hit = false;
+#pragma unroll 1
+                    for (int d = 0; d < 8; ++d) {
+                        if (((src[d] >> bx) & 1u) == 0u) continue;
+                        ++my_trials;
+                        const uint32_t T = __ldg(thr + (size_t)(c - (uint32_t)(fire_dy(d) * W + fire_dx(d))) * 8 + d);
+                        hit |= fire_trial(fire_rnd(key_lo, key_hi, sim, t, c, d), T);
+                    }
+                    if (hit) fresh |= 1u << bx;
+                }
+                nxt[wi] = fresh;                      // always written: this ring slot held the ignitions of kmax + 1 steps ago
+                if (fresh) { any_new = 1; ny0 = min(ny0, y); ny1 = max(ny1, y); }
+            }
+            __syncthreads();
+            int still = any_new;
+            for (int idx = tid; idx < nwords; idx += nthr) {
+                const size_t wi = (size_t)ylo * Ww + idx;
+                const uint32_t f = __ldcg(nxt + wi);
+                if (f) burned[wi] |= f;
+                if (!still && active_word(prm, ring, nw, t + 1u, ylo + idx / Ww, idx % Ww)) still = 1;    // cells that keep burning
+            }
+            if (any_new) { atomicMin(&s_y0, ny0); atomicMax(&s_y1, ny1); }
+            burning = __syncthreads_or(still);
+            ++t;
+        }
+        {   // leave the whole ring all-zero for the next simulation
+            const int ylo = max(s_y0 - 1, 0), yhi = min(s_y1 + 1, H - 1);
+            const size_t lo = (size_t)ylo * Ww, n = (size_t)(yhi - ylo + 1) * Ww;
+            for (uint32_t r = 0; r < R1; ++r)
+                for (size_t w = tid; w < n; w += nthr) ring[(size_t)r * nw + lo + w] = 0u;
+        }
+        if (my_trials) atomicAdd(&s_trials, my_trials);
+        __syncthreads();
+        if (tid == 0) {
+            if (prm.out_steps) prm.out_steps[s] = t;
+            if (prm.out_trials) prm.out_trials[s] = s_trials;
+        }
+        __syncthreads();
+    }
+}
+
+// fire_set_burn_time: per-cell burn time - 1 from the vegetation class, and the bitmaps "burn time > j + 1" of the rescue kernel
+struct burn_table { uint8_t k[256]; };
+__global__ void __launch_bounds__(256)
+fire_ktime_kernel(const uint8_t* __restrict__ veg, const burn_table tab, int W, int H, int Ww, int kmax, uint8_t* __restrict__ ktime,
+                  uint32_t* __restrict__ gt_planes)
+{
+    const size_t warp = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;      // one warp per bitmap word
+    const int lane = threadIdx.x & 31;
+    const size_t nw = (size_t)H * Ww;
+    if (warp >= nw) return;
+    const int y = (int)(warp / Ww), x = (int)(warp % Ww) * 32 + lane;
+    uint32_t k1 = 0u;
+    if (x < W) {
+        const size_t c = (size_t)y * W + x;
+        const uint8_t v = veg[c];
+        k1 = v ? (uint32_t)tab.k[v] - 1u : 0u;
+        ktime[c] = (uint8_t)k1;
+    }
+    for (int j = 1; j < kmax; ++j) {
+        const uint32_t word = __ballot_sync(0xFFFFFFFFu, k1 >= (uint32_t)j);            // burn time > j
+        if (lane == 0) gt_planes[(size_t)(j - 1) * nw + warp] = word;
+    }
+}
+
 constexpr int kRescueCtas = 16;
 
 }  // namespace
@@ -1055,6 +1233,38 @@ extern "C" int fire_set_schedule(fire_landscape* L, int32_t mode)
 {
     if (L == nullptr || mode < 0) return FIRE_EINVAL;
     L->schedule = mode & 1;
+    return FIRE_OK;
+}
+
+extern "C" int fire_set_burn_time(fire_landscape* L, const uint8_t* burn_time_host, int32_t n_classes, void* stream)
+{
+    if (L == nullptr || n_classes < 0 || n_classes > 256 || (n_classes > 0 && burn_time_host == nullptr)) return FIRE_EINVAL;
+    if (L->sticky) return L->sticky;
+    burn_table tab;
+    int kmax = 1;
+    for (int v = 0; v < 256; ++v) {
+        int k = v < n_classes ? (int)burn_time_host[v] : 1;
+        if (k == 0) k = 1;
+        if (k > 8) return FIRE_EINVAL;
+        tab.k[v] = (uint8_t)k;
+        if (v > 0 && k > kmax) kmax = k;
+    }
+    if (kmax == 1) { L->burn_kmax = 1; return FIRE_OK; }          // the base model: nothing to keep
+    fire_device_guard g(L->device);
+    if (!g.ok) return FIRE_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nw = (size_t)L->H * L->Ww;
+    if (L->ktime == nullptr || L->gt_capacity < nw * 4 * 7) {
+        FIRE_CUDA_TRY(L, cudaStreamSynchronize(st));
+        size_t cap = 0;
+        if (L->ktime == nullptr) { int rc = fire_reserve(L, (void**)&L->ktime, &cap, L->cells); if (rc != FIRE_OK) return rc; }
+        int rc = fire_reserve(L, (void**)&L->gt_planes, &L->gt_capacity, nw * 4 * 7);
+        if (rc != FIRE_OK) return rc;
+    }
+    fire_ktime_kernel<<<(unsigned)((nw * 32 + 255) / 256), 256, 0, st>>>(L->veg_class, tab, L->W, L->H, L->Ww, kmax, L->ktime, L->gt_planes);
+    FIRE_CUDA_TRY(L, cudaGetLastError());
+    L->launches += 1;
+    L->burn_kmax = kmax;
     return FIRE_OK;
 }
 
@@ -1094,8 +1304,10 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     // kernel (two state planes, one barrier per step, per-warp trial rings), 3 / 4 = the same as thread-block clusters of 2 / 4
     // CTAs per simulation; 0 = the two-phase kernel for batches that fill the GPU with 256-thread CTAs, the asynchronous-warp
     // kernel for small batches of large fires (wide CTAs, long fronts), as clusters when the batch is smaller than half the GPU
-    const bool async = L->kernel_family >= 2 || (L->kernel_family == 0 && threads >= 512 && L->threads_per_cta == 0);
-    int cluster = L->kernel_family == 3 ? 2 : (L->kernel_family == 4 ? 4 : 1);
+    // fuel-dependent burn-out times (fire_set_burn_time) are a variant of the two-phase kernel only
+    const bool bt = L->burn_kmax > 1;
+    const bool async = !bt && (L->kernel_family >= 2 || (L->kernel_family == 0 && threads >= 512 && L->threads_per_cta == 0));
+    int cluster = !async ? 1 : (L->kernel_family == 3 ? 2 : (L->kernel_family == 4 ? 4 : 1));
     if (L->kernel_family == 0 && async && threads == 1024)
         cluster = (long long)S * 4 <= L->num_sms ? 4 : ((long long)S * 2 <= L->num_sms ? 2 : 1);
     const long long resident = (long long)L->num_sms * per_sm / cluster;         // simulations in flight
@@ -1133,7 +1345,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     if (spill_per_list_set * spill_sets >= ((size_t)1 << 32)) return FIRE_EINVAL;   // spill slots are addressed by 32-bit word offsets
     const size_t nw = (size_t)L->H * L->Ww;
     const size_t nt = (size_t)L->Tw * L->Th;
-    const size_t rescue_bytes = nw * 4 * 2 * kRescueCtas;
+    const size_t rescue_bytes = nw * 4 * (bt ? (size_t)L->burn_kmax + 1 : 2) * kRescueCtas;
     if (nt * (size_t)S * planes >= ((size_t)1 << 31)) return FIRE_EINVAL;   // planes are addressed by 32-bit tile offsets: split the batch
     const size_t tiles_bytes = nt * 8 * (size_t)S * planes;
     if (L->status_capacity < (size_t)2 * S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes ||
@@ -1152,7 +1364,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
         if (L->rescue_capacity < rescue_bytes) {
             rc = fire_reserve(L, (void**)&L->rescue_planes, &L->rescue_capacity, rescue_bytes);
             if (rc != FIRE_OK) return rc;
-            FIRE_CUDA_TRY(L, cudaMemsetAsync(L->rescue_planes, 0, rescue_bytes, st));
+            FIRE_CUDA_TRY(L, cudaMemsetAsync(L->rescue_planes, 0, L->rescue_capacity, st));
         }
         if (L->burnable_tiles == nullptr) {
             size_t cap = 0;
@@ -1171,6 +1383,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     prm.work_counter = L->work_counter; prm.rescue_list = L->status; prm.spill = L->spill;
     prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.Tw = L->Tw; prm.Th = L->Th; prm.num_sms = L->num_sms;
     prm.max_steps = max_steps;
+    prm.ktime = bt ? L->ktime : nullptr; prm.gt_planes = bt ? L->gt_planes : nullptr; prm.kmax = bt ? L->burn_kmax : 1;
 
     // ---- launch order: largest expected fires first (only matters when there are more simulations than resident ones)
     prm.order = nullptr;
@@ -1197,6 +1410,8 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     void (*kernel)(const prop_params) = nullptr;
     if (async && cluster > 1) kernel = threads <= 256 ? fire_propagate_async_kernel<256, 4, true> : (threads <= 512 ? fire_propagate_async_kernel<512, 2, true> : fire_propagate_async_kernel<1024, 1, true>);
     else if (async) kernel = threads <= 256 ? fire_propagate_async_kernel<256, 4, false> : (threads <= 512 ? fire_propagate_async_kernel<512, 2, false> : fire_propagate_async_kernel<1024, 1, false>);
+    else if (bt) kernel = threads <= 256 ? fire_propagate_kernel<256, 4, 2, 4, true>
+                                         : (threads <= 512 ? fire_propagate_kernel<512, 2, 2, 4, true> : fire_propagate_kernel<1024, 1, 2, 4, true>);
     else kernel = threads <= 256 ? (per_sm <= 4 ? fire_propagate_kernel<256, 4, 2, 4> : fire_propagate_kernel<256, 8, 1, 2>)
                                  : (threads <= 512 ? fire_propagate_kernel<512, 2, 2, 4> : fire_propagate_kernel<1024, 1, 2, 4>);
     if (smem + 1024 > 48 * 1024)                     // dynamic + static shared memory beyond the default limit
@@ -1227,7 +1442,8 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
                                                                                           L->H, L->Ww, L->Tw, L->Th, S);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
-    fire_propagate_rescue_kernel<<<kRescueCtas, 256, 0, st>>>(prm, L->rescue_planes);
+    if (bt) fire_propagate_rescue_bt_kernel<<<kRescueCtas, 256, 0, st>>>(prm, L->rescue_planes);
+    else fire_propagate_rescue_kernel<<<kRescueCtas, 256, 0, st>>>(prm, L->rescue_planes);
     FIRE_CUDA_TRY(L, cudaGetLastError());
     L->launches += 4;
     return FIRE_OK;

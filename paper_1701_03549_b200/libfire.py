@@ -21,7 +21,7 @@ FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
     "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
-    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_error_string",
+    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
 
@@ -60,6 +60,7 @@ def load() -> C.CDLL:
     lib.fire_set_list_capacity.argtypes = [_vp, C.c_int32, C.c_int32]
     lib.fire_set_schedule.argtypes = [_vp, C.c_int32]
     lib.fire_set_kernel.argtypes = [_vp, C.c_int32]
+    lib.fire_set_burn_time.argtypes = [_vp, _vp, C.c_int32, _vp]
     lib.fire_set_profiling.argtypes = [_vp, C.c_int32]
     lib.fire_profile_read.argtypes = [_vp, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
     lib.fire_error_string.argtypes = [C.c_int]
@@ -235,6 +236,13 @@ def fire_set_launch_geometry(L: Landscape, threads_per_cta: int = 0, ctas_per_sm
 
 def fire_set_schedule(L: Landscape, mode: int = 0) -> None:
     _check(load().fire_set_schedule(L.handle, int(mode)), "fire_set_schedule")
+
+
+def fire_set_burn_time(L: Landscape, burn_time, stream=None) -> None:
+    """burn_time: sequence of steps per vegetation class (1..8), or None / empty for the base model."""
+    import numpy as np
+    bt = np.ascontiguousarray(np.asarray(burn_time if burn_time is not None else [], dtype=np.uint8))
+    _check(load().fire_set_burn_time(L.handle, bt.ctypes.data if bt.size else None, int(bt.size), _stream(stream)), "fire_set_burn_time")
 
 
 def fire_set_kernel(L: Landscape, family: int = 0) -> None:

@@ -584,6 +584,65 @@ def test_unknown_ignition_search_as_the_paper_runs_it(request):
     L.close()
 
 
+def test_burn_out_time_variant_matches_the_oracle(orc, request):
+    """fuel-dependent burn-out times 1..8 per vegetation class.  Random lattices, burn-time
+    tables, step limits, CTA sizes, list capacities (down to the global spill and the rescue kernel of this variant); the oracle
+    is fed the GPU's own threshold tables, so burnt maps, steps and trial counts must be bit-exact.  Setting all ones afterwards
+    is the base model again."""
+    rng = np.random.default_rng(20261105)
+    n = 0
+    for it in range(40):
+        H, W = int(rng.integers(1, 120)), int(rng.integers(1, 160))
+        ls = small_landscape(rng, H, W, nonburn=0.15)
+        P, S = int(rng.integers(1, 4)), int(rng.integers(1, 30))
+        betas = np.stack([[rng.uniform(-3.0, 0.0), rng.uniform(-1, 0), rng.uniform(-.5, .5), rng.uniform(0, 2), rng.uniform(0, 1.5)]
+                          for _ in range(P)]).astype(np.float32)
+        ign = np.stack([rng.integers(-1, W + 1, S), rng.integers(-1, H + 1, S)], 1).astype(np.int32)
+        par = rng.integers(0, P, S).astype(np.int32)
+        seeds = rng.integers(0, 2 ** 63, S).astype(np.uint64)
+        max_steps = int(rng.choice([0, 0, 0, 4, 23]))
+        bt = [1] + [int(v) for v in rng.integers(1, 9, 3)]
+        if it % 7 == 0:
+            bt = [1, 8, 1, 2]
+        geom = (int(rng.choice([32, 64, 128, 256, 512, 1024])), int(rng.integers(1, 5)))
+        caps = (int(rng.choice([0, 0, 1, 4, 16])), int(rng.choice([0, 0, 0, 2, 64])))
+        Lo = orc_landscape(orc, ls)
+        L = gh.make_landscape(ls)
+        gh.upload(L, betas)
+        tables = [gh.thresholds(L, p) for p in range(P)]
+        lf.fire_set_launch_geometry(L, *geom)
+        lf.fire_set_list_capacity(L, *caps)
+        lf.fire_set_kernel(L, int(rng.choice([0, 1, 2])))             # the variant runs on the two-phase kernel whatever is asked
+        lf.fire_set_burn_time(L, bt)
+        g = gh.simulate(L, ign, par, seeds, max_steps=max_steps)
+        what = (it, H, W, P, S, max_steps, bt, geom, caps)
+        for s_ in range(S):
+            if 0 <= par[s_] < P:
+                o = orc.simulate_burn_time(Lo, betas[par[s_]], bt, ign[s_], int(seeds[s_]), sim=s_, max_steps=max_steps, table=tables[par[s_]])
+                assert (g["burned"][s_] == o["burned"]).all(), (what, s_)
+                assert g["steps"][s_] == o["steps"] and int(g["trials"][s_]) == o["trials"], (what, s_, g["steps"][s_], o["steps"])
+        if it % 5 == 0:                                               # back to one step everywhere: the base model, bit for bit
+            lf.fire_set_burn_time(L, [1, 1, 1, 1])
+            g1 = gh.simulate(L, ign, par, seeds, max_steps=max_steps)
+            o1 = orc.simulate_batch(Lo, betas, ign, par, seeds, max_steps=max_steps, tables=tables)
+            assert (g1["burned"] == o1["burned"]).all() and (g1["steps"] == o1["steps"]).all() and (g1["trials"] == o1["trials"]).all(), what
+        n += 1
+        L.close()
+    # config 2 at full size with burn times (forest 3 steps, the other classes 1-2): every sim against the oracle's own thresholds
+    w = wl.load_workload(2)
+    Lo = orc_landscape(orc, w.landscape); L = gh.make_landscape(w.landscape)
+    gh.upload(L, w.betas)
+    bt = [1, 3, 2, 1]
+    lf.fire_set_burn_time(L, bt)
+    g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    idx = np.arange(0, w.S, 8)
+    for s_ in idx:
+        o = orc.simulate_burn_time(Lo, w.betas[w.sim_param[s_]], bt, w.ignitions[s_], int(w.seeds[s_]), sim=int(s_))
+        assert (g["burned"][s_] == o["burned"]).all() and g["steps"][s_] == o["steps"] and int(g["trials"][s_]) == o["trials"], s_
+    report(request, cases=n, cfg2_sims_checked=len(idx), cfg2_trials=int(g["trials"].sum()))
+    L.close()
+
+
 # ---------------------------------------------------------------------------------- randomised parity
 def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
     """Seeded fuzz: random lattice sizes (1 x 1 .. 140 x 200, ragged), vegetation, parameters, ignitions (some off the lattice
