@@ -91,6 +91,15 @@ int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, const int32
                         const uint64_t* seeds, const int32_t* sim_ids, int32_t S, uint32_t max_steps,
                         uint32_t* out_burned, uint32_t* out_steps, uint64_t* out_trials, void* stream);
 
+/* Variant of the uphill test (PAPER.md:87 read literally): with an elevation raster f32[H][W] the slope term of
+ * direction d applies iff slope > 0 and elevation[target] > elevation[source] (strictly), source = target - offset(d), instead
+ * of the default local-plane test on the aspect (R-7).  Invalidates the threshold table: call fire_params_upload again. */
+int fire_landscape_set_elevation(fire_landscape* L, const float* elevation, void* stream);
+
+/* Hazard map: out_count u32[H][W] = number of the S maps burned u32[S][H][ceil(W/32)] in which the
+ * cell is burnt (divide by S for the burn probability of the cell over replicates). */
+int fire_burn_count(fire_landscape* L, const uint32_t* burned, int32_t S, uint32_t* out_count, void* stream);
+
 /* Fuel-dependent burn-out time ("a burnt cell gets inactive after a given time that depends on the
  * vegetation type", :145, :68, :273; reading R-21).  burn_time_host u8[n_classes] (HOST memory, read before the call
  * returns): steps a cell of vegetation class v stays ACTIVE once ignited, 1..8 (0 reads as 1; classes >= n_classes burn one

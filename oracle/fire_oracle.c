@@ -173,6 +173,37 @@ void orc_threshold_table(const float beta[5], const uint8_t* veg, const float* s
         }
 }
 
+/* Variant of C-2 / C-3 (PAPER.md:87 read literally): "Slope is calculated based on the digital elevation map (DEM)
+ * and is ignored whenever the target landscape cell is at a lower elevation or when slope is zero. The normalized slope is used
+ * when the target cell is higher in elevation than the burning cell."  With an elevation raster the uphill test of direction d
+ * is  elevation[target] > elevation[source]  (strictly, R-14), source = target - offset(d), instead of R-7's local-plane test on
+ * the aspect; everything else is orc_probability.  Entries whose source lies outside the lattice are never tried; they get
+ * sigma = 0. */
+void orc_threshold_table_dem(const float beta[5], const uint8_t* veg, const float* slope, const float* aspect,
+                             const float* wind, const float* elevation, int W, int H, uint32_t* out)
+{
+    double b0 = (double)beta[0], b1 = (double)beta[1], b2 = (double)beta[2], b3 = (double)beta[3], b4 = (double)beta[4];
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            size_t c = (size_t)y * W + x;
+            orc_cov cv;
+            orc_covariates(veg[c], slope[c], aspect[c], wind[c], &cv);
+            for (int d = 0; d < 8; ++d) {
+                int sx = x - DX[d], sy = y - DY[d];
+                int inside = sx >= 0 && sx < W && sy >= 0 && sy < H;
+                int uphill = inside && ((double)slope[c] > 0.0) && (elevation[c] > elevation[(size_t)sy * W + sx]);
+                double sigma = uphill ? tan((double)slope[c]) : 0.0;
+                double xx = b0 + b1 * cv.I_f;
+                xx = xx + b2 * cv.psi;
+                xx = xx + b3 * cv.omega[d];
+                xx = xx + b4 * sigma;
+                double p = 1.0 / (1.0 + exp(-xx));
+                long long t = llrint(ldexp(p, 32));
+                out[c * 8 + d] = cv.burnable ? (uint32_t)(t > 0xFFFFFFFFll ? 0xFFFFFFFFll : t) : 0u;
+            }
+        }
+}
+
 /* ------------------------------------------------------------------------- *
  * C-4: one simulation (PAPER.md:91 states; :97 ignition; :99, :133 synchronous
  * update, independent trial per burning neighbour = 1 - prod(1 - p_i) in law,

@@ -73,6 +73,8 @@ def _declare(l):
     l.orc_trial_succeeds.restype = C.c_int
     l.orc_threshold_table.argtypes = [_f32p, _u8p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _u32p]
     l.orc_threshold_table.restype = None
+    l.orc_threshold_table_dem.argtypes = [_f32p, _u8p, _f32p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _u32p]
+    l.orc_threshold_table_dem.restype = None
     l.orc_simulate.argtypes = [_u8p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _f32p, _u32p,
                                C.c_int, C.c_int, C.c_uint64, C.c_uint32, C.c_uint32,
                                _u32p, _i32p, _u32p, _u64p]
@@ -171,6 +173,23 @@ def threshold_table(L: Landscape, beta) -> np.ndarray:
     out = np.zeros((L.H, L.W, 8), np.uint32)
     lib().orc_threshold_table(_p(b, _f32p), *L._ptrs(), L.W, L.H, _p(out, _u32p))
     return out
+
+
+def threshold_table_dem(L: Landscape, beta, elevation) -> np.ndarray:
+    """Table with the literal DEM uphill test of PAPER.md:87 (variant f4): elevation f32[H][W]."""
+    b = _c(beta, np.float32)
+    z = _c(elevation, np.float32)
+    assert z.shape == (L.H, L.W)
+    out = np.zeros((L.H, L.W, 8), np.uint32)
+    lib().orc_threshold_table_dem(_p(b, _f32p), *L._ptrs(), _p(z, _f32p), L.W, L.H, _p(out, _u32p))
+    return out
+
+
+def burn_count(burned_batch, W: int) -> np.ndarray:
+    """Hazard map (the use of [12]): for every cell, in how many of the maps it is burnt.  u32[H][W]."""
+    b = np.ascontiguousarray(burned_batch, dtype="<u4")
+    bits = np.unpackbits(b.view(np.uint8), axis=-1, bitorder="little")[..., :W]
+    return bits.sum(axis=0, dtype=np.uint32)
 
 
 # --------------------------------------------------------------------------- C-4

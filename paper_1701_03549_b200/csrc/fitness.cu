@@ -133,7 +133,51 @@ fire_group_stats_kernel(const uint32_t* __restrict__ counts, uint32_t N, int G, 
     }
 }
 
+// Hazard map (f4): per-cell number of maps in which the cell is burnt.  One thread per bitmap word and slab of maps:
+// the 32 counts of the word live in registers while the slab streams by (one coalesced 4 B load per map), then go to the output
+// with one integer atomic each.
+__global__ void __launch_bounds__(256)
+fire_burn_count_kernel(const uint32_t* __restrict__ burned, size_t nw, int W, int Ww, int S, int slab, uint32_t* __restrict__ out)
+{
+    const size_t wi = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (wi >= nw) return;
+    const int s0 = blockIdx.y * slab, s1 = min(S, s0 + slab);
+    uint32_t cnt[32];
+#pragma unroll
+    for (int b = 0; b < 32; ++b) cnt[b] = 0u;
+    for (int s = s0; s < s1; ++s) {
+        const uint32_t w = __ldcs(burned + (size_t)s * nw + wi);
+#pragma unroll
+        for (int b = 0; b < 32; ++b) cnt[b] += (w >> b) & 1u;
+    }
+    const int y = (int)(wi / Ww), x0 = (int)(wi % Ww) * 32;
+#pragma unroll
+    for (int b = 0; b < 32; ++b)
+        if (x0 + b < W && cnt[b]) atomicAdd(out + (size_t)y * W + x0 + b, cnt[b]);
+}
+
 }  // namespace
+
+extern "C" int fire_burn_count(fire_landscape* L, const uint32_t* burned, int32_t S, uint32_t* out_count, void* stream)
+{
+    if (L == nullptr || burned == nullptr || out_count == nullptr || S < 1) return FIRE_EINVAL;
+    if (L->sticky) return L->sticky;
+    fire_device_guard g(L->device);
+    if (!g.ok) return FIRE_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nw = (size_t)L->H * L->Ww;
+    FIRE_CUDA_TRY(L, cudaMemsetAsync(out_count, 0, L->cells * sizeof(uint32_t), st));
+    const int slab = 64;
+    const unsigned gy = (unsigned)((S + slab - 1) / slab);
+    for (unsigned y0 = 0; y0 < gy; y0 += 65535) {                           // gridDim.y <= 65535
+        const unsigned ny = gy - y0 < 65535 ? gy - y0 : 65535;
+        fire_burn_count_kernel<<<dim3((unsigned)((nw + 255) / 256), ny), 256, 0, st>>>(burned + (size_t)y0 * slab * nw, nw, L->W, L->Ww,
+                                                                                       S - (int)(y0 * slab), slab, out_count);
+        FIRE_CUDA_TRY(L, cudaGetLastError());
+        L->launches += 1;
+    }
+    return FIRE_OK;
+}
 
 extern "C" int fire_fitness(fire_landscape* L, const uint32_t* reference, const uint32_t* burned, int32_t S,
                             int32_t metric, float* out_score, uint32_t* out_counts, uint32_t* out_ref_area, void* stream)

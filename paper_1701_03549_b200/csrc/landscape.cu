@@ -318,7 +318,41 @@ fire_thresholds_gather_kernel(const float* __restrict__ beta5, int W, int H,
     out[i] = T;
 }
 
+// f4 variant (PAPER.md:87 read literally): uphill in direction d <=> slope > 0 and elevation[target] > elevation[source],
+// source = target - offset(d) inside the lattice; replaces the aspect-based mask written by fire_covariates_kernel.
+__global__ void __launch_bounds__(256)
+fire_uphill_from_dem_kernel(const float* __restrict__ elevation, const double* __restrict__ tan_slope, int W, int H,
+                            uint8_t* __restrict__ uphill)
+{
+    const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= (size_t)W * H) return;
+    const int x = (int)(c % W), y = (int)(c / W);
+    uint32_t up = 0u;
+    if (tan_slope[c] > 0.0) {                                              // tan(s) > 0 <=> s > 0 on [0, pi/2)
+        const float z = elevation[c];
+#pragma unroll
+        for (int d = 0; d < 8; ++d) {
+            const int sx = x - fire_dx(d), sy = y - fire_dy(d);
+            if (sx >= 0 && sx < W && sy >= 0 && sy < H && z > elevation[(size_t)sy * W + sx]) up |= 1u << d;
+        }
+    }
+    uphill[c] = (uint8_t)up;
+}
+
 }  // namespace
+
+extern "C" int fire_landscape_set_elevation(fire_landscape* L, const float* elevation, void* stream)
+{
+    if (L == nullptr || elevation == nullptr) return FIRE_EINVAL;
+    if (L->sticky) return L->sticky;
+    fire_device_guard g(L->device);
+    if (!g.ok) return FIRE_ECUDA;
+    fire_uphill_from_dem_kernel<<<(unsigned)((L->cells + 255) / 256), 256, 0, (cudaStream_t)stream>>>(elevation, L->tan_slope, L->W, L->H, L->uphill);
+    FIRE_CUDA_TRY(L, cudaGetLastError());
+    L->launches += 1;
+    L->P = 0;                                                              // any table built before is stale
+    return FIRE_OK;
+}
 
 // ----------------------------------------------------------------------------------------------
 extern "C" int fire_landscape_destroy(fire_landscape* L)

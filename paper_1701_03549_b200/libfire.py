@@ -21,7 +21,7 @@ FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
     "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
-    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_error_string",
+    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_landscape_set_elevation", "fire_burn_count", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
 
@@ -61,6 +61,8 @@ def load() -> C.CDLL:
     lib.fire_set_schedule.argtypes = [_vp, C.c_int32]
     lib.fire_set_kernel.argtypes = [_vp, C.c_int32]
     lib.fire_set_burn_time.argtypes = [_vp, _vp, C.c_int32, _vp]
+    lib.fire_landscape_set_elevation.argtypes = [_vp, _vp, _vp]
+    lib.fire_burn_count.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     lib.fire_set_profiling.argtypes = [_vp, C.c_int32]
     lib.fire_profile_read.argtypes = [_vp, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
     lib.fire_error_string.argtypes = [C.c_int]
@@ -236,6 +238,17 @@ def fire_set_launch_geometry(L: Landscape, threads_per_cta: int = 0, ctas_per_sm
 
 def fire_set_schedule(L: Landscape, mode: int = 0) -> None:
     _check(load().fire_set_schedule(L.handle, int(mode)), "fire_set_schedule")
+
+
+def fire_landscape_set_elevation(L: Landscape, elevation: torch.Tensor, stream=None) -> None:
+    _check(load().fire_landscape_set_elevation(L.handle, _dev(elevation, torch.float32, "elevation", (L.H, L.W)), _stream(stream)),
+           "fire_landscape_set_elevation")
+
+
+def fire_burn_count(L: Landscape, burned: torch.Tensor, out_count: torch.Tensor, stream=None) -> None:
+    S = int(burned.shape[0])
+    _check(load().fire_burn_count(L.handle, _dev(burned, torch.int32, "burned", (S, L.H, L.Ww)), S,
+                                  _dev(out_count, torch.int32, "out_count", (L.H, L.W)), _stream(stream)), "fire_burn_count")
 
 
 def fire_set_burn_time(L: Landscape, burn_time, stream=None) -> None:

@@ -21,7 +21,9 @@ typedef int (*profread_fn)(fire_landscape*, float*, int32_t, int32_t*);
 typedef const char* (*errstr_fn)(int);
 
 typedef int (*burn_fn)(fire_landscape*, const uint8_t*, int32_t, void*);
-any_fn fire_abi_table[17];
+typedef int (*elev_fn)(fire_landscape*, const float*, void*);
+typedef int (*hazard_fn)(fire_landscape*, const uint32_t*, int32_t, uint32_t*, void*);
+any_fn fire_abi_table[19];
 
 void fire_abi_fill(void)
 {
@@ -34,7 +36,9 @@ void fire_abi_fill(void)
     set1_fn f12 = fire_set_kernel;              set1_fn f13 = fire_set_profiling;
     profread_fn f14 = fire_profile_read;        errstr_fn f15 = fire_error_string;
     burn_fn f16 = fire_set_burn_time;
-    fire_abi_table[16] = (any_fn)f16;
+    elev_fn f17 = fire_landscape_set_elevation;
+    hazard_fn f18 = fire_burn_count;
+    fire_abi_table[16] = (any_fn)f16; fire_abi_table[17] = (any_fn)f17; fire_abi_table[18] = (any_fn)f18;
     fire_abi_table[0] = (any_fn)f0;   fire_abi_table[1] = (any_fn)f1;
     fire_abi_table[2] = (any_fn)f2;   fire_abi_table[3] = (any_fn)f3;
     fire_abi_table[4] = (any_fn)f4;   fire_abi_table[5] = (any_fn)f5;

@@ -643,6 +643,43 @@ def test_burn_out_time_variant_matches_the_oracle(orc, request):
     L.close()
 
 
+def test_dem_uphill_variant_and_hazard_map(orc, request):
+    """(i) the literal DEM uphill test of PAPER.md:87 (fire_landscape_set_elevation) -- thresholds within one count of
+    the oracle's table, propagation bit-exact on the GPU's table; (ii) the hazard map of PAPER.md:54 (fire_burn_count) equals the
+    per-cell sum over the burnt maps, including a ragged width and more maps than one slab."""
+    rng = np.random.default_rng(77)
+    n_diff = 0
+    for H, W in [(40, 50), (33, 77), (64, 64)]:
+        ls = small_landscape(rng, H, W)
+        z = (np.cumsum(rng.standard_normal((H, W)), axis=1) * 5 + 200).astype(np.float32)
+        betas = np.array([[-0.8, -0.4, 0.3, 0.9, 1.2], [-1.5, 0.2, -0.1, 1.4, 0.4]], np.float32)
+        Lo = orc_landscape(orc, ls); L = gh.make_landscape(ls)
+        lf.fire_landscape_set_elevation(L, gh.dev(z))
+        gh.upload(L, betas)
+        tabs = []
+        for p in range(2):
+            g = gh.thresholds(L, p); o = orc.threshold_table_dem(Lo, betas[p], z)
+            # entries whose source lies outside the lattice are never tried: the test hook evaluates them with sigma = 0 as well
+            d = np.abs(g.astype(np.int64) - o.astype(np.int64))
+            assert d.max() <= 1, (H, W, p, d.max())
+            n_diff += int((d != 0).sum()); tabs.append(g)
+        base = orc.threshold_table(Lo, betas[0])
+        assert (tabs[0] != base).any()                                # the variant really changes the table
+        S = 150
+        ign = np.stack([rng.integers(0, W, S), rng.integers(0, H, S)], 1).astype(np.int32)
+        par = rng.integers(0, 2, S).astype(np.int32); seeds = rng.integers(0, 2 ** 63, S).astype(np.uint64)
+        g = gh.simulate(L, ign, par, seeds, keep_device=True)
+        o = orc.simulate_batch(Lo, betas, ign, par, seeds, tables=tabs)
+        gb = g["burned"].cpu().numpy().view(np.uint32)
+        assert (gb == o["burned"]).all() and (g["steps"] == o["steps"]).all() and (g["trials"] == o["trials"]).all()
+        count = torch.full((H, W), -1, dtype=torch.int32, device="cuda")
+        lf.fire_burn_count(L, g["burned"], count)
+        torch.cuda.synchronize()
+        assert (count.cpu().numpy().view(np.uint32) == orc.burn_count(o["burned"], W)).all()
+        L.close()
+    report(request, one_count_differences=n_diff)
+
+
 # ---------------------------------------------------------------------------------- randomised parity
 def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
     """Seeded fuzz: random lattice sizes (1 x 1 .. 140 x 200, ragged), vegetation, parameters, ignitions (some off the lattice
