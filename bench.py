@@ -401,21 +401,31 @@ def run_ours(args) -> None:
     alg_bytes = 32 * int(np.array(golden["distinct"], np.int64)[l_index].sum()) + 2 * plane_bytes * S
     k_ms = float(np.mean(prop_ms)) if prop_ms else float("nan")
     achieved = alg_bytes / (k_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "fire_propagate_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    # which propagation kernel fire_simulate_batch picks by default (propagate.cu, fire_simulate_batch: geometry and family)
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
+    if S >= 2 * sms or L.W * L.H < 2048 * 2048:
+        kname = "fire_propagate_kernel (two-phase, one CTA per simulation)"
+    elif 2 * S <= sms:
+        kname = f"fire_propagate_async_kernel (clusters of {4 if 4 * S <= sms else 2} CTAs per simulation)"
+    else:
+        kname = "fire_propagate_async_kernel (one CTA per simulation)"
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get(cfg) if world == 1 else None,
                 "traffic_source": NCU_TRAFFIC_SOURCE.get(cfg) if world == 1 else None, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms, "launches_timed": len(prop_ms),
                 "share_of_step": k_ms / ms_per_step,
                 "philox_calls_per_s": trials_rank / (k_ms * 1e-3)}
-    # second ceiling: the kernel is issue-bound, not HBM-bound.  Algorithmic integer work = one
-    # Philox4x32-10 call per trial = 20 wide multiplies + 20 three-input xors = 40 lane operations; peak = SMs x 4 schedulers
-    # x 32 lanes x max SM clock, one instruction per scheduler per clock.
+    # second ceiling: the arithmetic the method cannot avoid is one Philox4x32-10 call per trial = 18 wide
+    # multiplies (IMAD.WIDE.U32; rounds 0 and 1 share their products over a step) + 18 three-input xors.  The wide multiplies run
+    # on the FMA-heavy pipe only, one warp instruction per 4 cycles per SM sub-partition (measured: sm__pipe_fmaheavy_cycles_active
+    # against the executed IMAD mix, profiles/r2_propagate_ncu.md), so peak = SMs x 4 sub-partitions x clock x 32 lanes / (18 x 4).
     sm_count = torch.cuda.get_device_properties(local).multi_processor_count
     sm_clock_hz = 1e6 * float((clocks or {}).get("sm_max_mhz") or 1965.0)
-    alu_peak = sm_count * 4 * 32 * sm_clock_hz
-    alu_ach = 40.0 * trials_rank / (k_ms * 1e-3)
-    roofline["alu"] = {"bound": "alu", "achieved": alu_ach / 1e12, "peak": alu_peak / 1e12, "unit": "Tera lane-ops/s",
-                       "frac": alu_ach / alu_peak, "note": "40 lane-ops per trial (Philox4x32-10) / issue peak"}
+    alu_peak = sm_count * 4 * sm_clock_hz * 32 / (18 * 4)
+    alu_ach = trials_rank / (k_ms * 1e-3)
+    roofline["alu"] = {"bound": "alu", "achieved": alu_ach / 1e9, "peak": alu_peak / 1e9, "unit": "G Philox calls/s",
+                       "frac": alu_ach / alu_peak,
+                       "note": "18 IMAD.WIDE per Philox4x32-10 call on the FMA-heavy pipe at 1 per 4 cycles per SM sub-partition"}
 
     # ---- CPU baseline: the oracle as it stands on a bounded sample of the same workload
     cpu = None

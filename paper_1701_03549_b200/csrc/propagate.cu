@@ -1303,10 +1303,15 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     // kernel family (fire_set_kernel): 1 = two-phase kernel (one state plane, two block barriers per step), 2 = asynchronous-warp
     // kernel (two state planes, one barrier per step, per-warp trial rings), 3 / 4 = the same as thread-block clusters of 2 / 4
     // CTAs per simulation; 0 = the two-phase kernel for batches that fill the GPU with 256-thread CTAs, the asynchronous-warp
-    // kernel for small batches of large fires (wide CTAs, long fronts), as clusters when the batch is smaller than half the GPU
+    // kernel for small batches of large fires (wide CTAs, lattices of 2048 x 2048 or more), as clusters when the batch is smaller
+    // than half the GPU
     // fuel-dependent burn-out times (fire_set_burn_time) are a variant of the two-phase kernel only
     const bool bt = L->burn_kmax > 1;
-    const bool async = !bt && (L->kernel_family >= 2 || (L->kernel_family == 0 && threads >= 512 && L->threads_per_cta == 0));
+    // (measured on one simulation of config 3 alone on the GPU: 2.6 us per step with the two-phase kernel at 1024 threads, 3.2 with
+    // the asynchronous-warp kernel, 5.0-5.6 as a cluster -- a cluster barrier costs about 2 us; on config 5, whose fronts are
+    // thousands of cells long, 89.6 / 85.0 / 64.2 ms: the wide families pay off on large lattices only)
+    const bool big_lattice = L->cells >= (size_t)2048 * 2048;
+    const bool async = !bt && (L->kernel_family >= 2 || (L->kernel_family == 0 && threads >= 512 && L->threads_per_cta == 0 && big_lattice));
     int cluster = !async ? 1 : (L->kernel_family == 3 ? 2 : (L->kernel_family == 4 ? 4 : 1));
     if (L->kernel_family == 0 && async && threads == 1024)
         cluster = (long long)S * 4 <= L->num_sms ? 4 : ((long long)S * 2 <= L->num_sms ? 2 : 1);
