@@ -100,6 +100,12 @@ int fire_landscape_set_elevation(fire_landscape* L, const float* elevation, void
  * cell is burnt (divide by S for the burn probability of the cell over replicates). */
 int fire_burn_count(fire_landscape* L, const uint32_t* burned, int32_t S, uint32_t* out_count, void* stream);
 
+/* Time-of-burn output ("fire evolution in time"): out_time i32[S][H][W] (device; the caller's, sized
+ * for the largest batch it will pass) receives, in every later fire_simulate_batch on this handle, the step at which each cell
+ * ignited: 0 for the ignition cell, t + 1 for a cell ignited by the transition t -> t + 1, -1 for a cell that never burnt.
+ * NULL switches the output off (default). */
+int fire_set_time_output(fire_landscape* L, int32_t* out_time);
+
 /* Fuel-dependent burn-out time ("a burnt cell gets inactive after a given time that depends on the
  * vegetation type", :145, :68, :273; reading R-21).  burn_time_host u8[n_classes] (HOST memory, read before the call
  * returns): steps a cell of vegetation class v stays ACTIVE once ignited, 1..8 (0 reads as 1; classes >= n_classes burn one

@@ -55,6 +55,7 @@ struct fire_landscape {
     uint32_t* gt_planes;          // [7][H][Ww] bit set iff burn time > j + 1
     size_t    gt_capacity;
     int       burn_kmax;          // largest burn time set; <= 1 = the base model (every cell burns one step)
+    int32_t*  out_time;           // fire_set_time_output: the caller's [S][H][W] ignition-time array, or null
 
     // a7: fitness scratch
     uint32_t* ref_area;           // [1]

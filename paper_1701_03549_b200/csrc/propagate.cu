@@ -54,6 +54,7 @@ struct prop_params {
     const uint8_t* ktime;         // [cells] burn time - 1 of the cell's fuel (fire_set_burn_time), or null
     const uint32_t* gt_planes;    // [kmax - 1][H][Ww] bit set iff the cell's burn time > j + 1 (rescue kernel), or null
     int kmax;                     // largest burn time (1 = every cell burns for one step)
+    int32_t* out_time;            // [S][H][W] step at which every cell ignited (fire_set_time_output), or null
 };
 
 __device__ __forceinline__ uint32_t lanemask_lt()
@@ -144,6 +145,8 @@ struct step_ctx {
     uint32_t nA, nQ;
     uint32_t lane, lt;
     const uint8_t* ktime;         // burn-time variant only
+    int32_t* time_base;           // burn-time variant only: ignition times of this simulation, or null
+    uint32_t t;                   // burn-time variant only: the step being computed
 };
 
 // Appends `entry` of the lanes with `flag` to the next frontier list (shared memory, then the global spill, then overflow).
@@ -357,7 +360,11 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
             uint32_t en = pt.item[u] & 0xFFFF1FFFu;
             const uint32_t a = c.an_addr + 4u * (abase + __popc(fresh_mask[u] & c.lt));
             if (fresh_mask[u] & (1u << c.lane)) {
-                if (kBT) en |= (uint32_t)__ldg(c.ktime + ((en >> 16) * c.W + (en & 0x1FFFu))) << 29;      // burn time of its fuel - 1
+                if (kBT) {
+                    const uint32_t cell = (en >> 16) * c.W + (en & 0x1FFFu);
+                    if (c.time_base) c.time_base[cell] = (int32_t)(c.t + 1u);                              // ignited by the transition t -> t + 1
+                    en |= (uint32_t)__ldg(c.ktime + cell) << 29;                                           // burn time of its fuel - 1
+                }
                 sts32(a, en);
             }
             abase += __popc(fresh_mask[u]);
@@ -368,7 +375,11 @@ __device__ __forceinline__ void trials_resolve(const step_ctx& c, const pending_
             if (fresh_mask[u] & (1u << c.lane)) {
                 const uint32_t pos = abase + __popc(fresh_mask[u] & c.lt);
                 uint32_t en = pt.item[u] & 0xFFFF1FFFu;
-                if (kBT) en |= (uint32_t)__ldg(c.ktime + ((en >> 16) * c.W + (en & 0x1FFFu))) << 29;
+                if (kBT) {
+                    const uint32_t cell = (en >> 16) * c.W + (en & 0x1FFFu);
+                    if (c.time_base) c.time_base[cell] = (int32_t)(c.t + 1u);
+                    en |= (uint32_t)__ldg(c.ktime + cell) << 29;
+                }
                 if (pos < c.capA_s) sts32(c.an_addr + 4u * pos, en);
                 else if (pos < c.capA) __stcg(c.spill + (c.an_off + (pos - c.capA_s)), en);
                 else sts32(c.over, 1u);
@@ -436,7 +447,7 @@ fire_propagate_kernel(const prop_params prm)
     const uint32_t cntQ_addr = cntA_addr + 8u;
     c.over = cntA_addr + 16u;
     c.lane = (uint32_t)tid & 31u; c.lt = lanemask_lt();
-    c.ktime = prm.ktime;
+    c.ktime = prm.ktime; c.time_base = nullptr; c.t = 0u;
 
     for (;;) {
         __syncthreads();                       // the previous simulation's last reads of s_* are done
@@ -455,6 +466,7 @@ fire_propagate_kernel(const prop_params prm)
         bool valid = p >= 0 && p < prm.P && ix >= 0 && ix < prm.W && iy >= 0 && iy < prm.H;     // R-12
         if (valid) valid = (__ldg(prm.burnable + (size_t)iy * prm.Ww + (ix >> 5)) >> (ix & 31)) & 1u;
         c.thr_sec = valid ? (uint32_t)p * (c.W * (uint32_t)prm.H) : 0u;
+        if (kBT) c.time_base = prm.out_time ? prm.out_time + (size_t)s * ((size_t)prm.W * prm.H) : nullptr;
         // the key is the same in every lane: a warp reduction leaves it in a UNIFORM register, and so are the round keys
         // derived from it (they then cost no per-thread registers)
         const uint32_t key_lo = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)seed), key_hi = __reduce_or_sync(0xFFFFFFFFu, (uint32_t)(seed >> 32));
@@ -467,6 +479,7 @@ fire_propagate_kernel(const prop_params prm)
             if (valid) {
                 uint32_t e0 = ((uint32_t)iy << 16) | (uint32_t)ix;
                 if (kBT) e0 |= (uint32_t)prm.ktime[(size_t)iy * prm.W + ix] << 29;
+                if (kBT && c.time_base) c.time_base[(size_t)iy * prm.W + ix] = 0;
                 if (prm.capA_s > 0) sts32(as_addr0, e0); else prm.spill[ag_off0] = e0;
                 atomicAnd(reinterpret_cast<uint32_t*>(prm.tiles) + (((size_t)c.plane_w + (size_t)(iy >> 3) * c.Tw + (ix >> 3)) * 2 + ((iy >> 2) & 1)), ~(1u << (((iy & 3) << 3) | (ix & 7))));
             }
@@ -478,6 +491,7 @@ fire_propagate_kernel(const prop_params prm)
         bool over = false;
         while (c.nA > 0 && (prm.max_steps == 0 || t < prm.max_steps)) {
             const uint32_t par = t & 1u;
+            if (kBT) c.t = t;
             c.ac_addr = par ? as_addr1 : as_addr0; c.an_addr = par ? as_addr0 : as_addr1;
             c.ac_off = par ? ag_off1 : ag_off0; c.an_off = par ? ag_off0 : ag_off1;
             c.cntQ = cntQ_addr + 4u * par; c.cntA_next = cntA_addr + 4u * (par ^ 1u);
@@ -1100,11 +1114,13 @@ fire_propagate_rescue_bt_kernel(const prop_params prm, uint32_t* planes)
         uint32_t* const ring = planes + (size_t)blockIdx.x * R1 * nw;
 
         for (size_t w = tid; w < nw; w += nthr) burned[w] = 0u;      // the fast kernel left it half-done
+        if (prm.out_time) for (size_t c = tid; c < (size_t)W * H; c += nthr) prm.out_time[(size_t)s * W * H + c] = -1;
         if (tid == 0) { s_y0 = iy; s_y1 = iy; s_trials = 0ull; }
         __syncthreads();
         if (tid == 0) {
             burned[(size_t)iy * Ww + (ix >> 5)] = 1u << (ix & 31);
             ring[(size_t)iy * Ww + (ix >> 5)] = 1u << (ix & 31);      // ignited "by the transition into state 0"
+            if (prm.out_time) prm.out_time[(size_t)s * W * H + (size_t)iy * W + ix] = 0;
         }
         __syncthreads();
 
@@ -1149,7 +1165,10 @@ fire_propagate_rescue_bt_kernel(const prop_params prm, uint32_t* planes)
                         const uint32_t T = __ldg(thr + (size_t)(c - (uint32_t)(fire_dy(d) * W + fire_dx(d))) * 8 + d);
                         hit |= fire_trial(fire_rnd(key_lo, key_hi, sim, t, c, d), T);
                     }
-                    if (hit) fresh |= 1u << bx;
+                    if (hit) {
+                        fresh |= 1u << bx;
+                        if (prm.out_time) prm.out_time[(size_t)s * W * H + c] = (int32_t)(t + 1u);
+                    }
                 }
                 nxt[wi] = fresh;                      // always written: this ring slot held the ignitions of kmax + 1 steps ago
                 if (fresh) { any_new = 1; ny0 = min(ny0, y); ny1 = max(ny1, y); }
@@ -1268,6 +1287,13 @@ extern "C" int fire_set_burn_time(fire_landscape* L, const uint8_t* burn_time_ho
     return FIRE_OK;
 }
 
+extern "C" int fire_set_time_output(fire_landscape* L, int32_t* out_time)
+{
+    if (L == nullptr) return FIRE_EINVAL;
+    L->out_time = out_time;
+    return FIRE_OK;
+}
+
 extern "C" int fire_set_kernel(fire_landscape* L, int32_t family)
 {
     if (L == nullptr || family < 0 || family > 4) return FIRE_EINVAL;
@@ -1306,7 +1332,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     // kernel for small batches of large fires (wide CTAs, lattices of 2048 x 2048 or more), as clusters when the batch is smaller
     // than half the GPU
     // fuel-dependent burn-out times (fire_set_burn_time) are a variant of the two-phase kernel only
-    const bool bt = L->burn_kmax > 1;
+    const bool bt = L->burn_kmax > 1 || L->out_time != nullptr;         // ignition times are written by the same variant
     // (measured on one simulation of config 3 alone on the GPU: 2.6 us per step with the two-phase kernel at 1024 threads, 3.2 with
     // the asynchronous-warp kernel, 5.0-5.6 as a cluster -- a cluster barrier costs about 2 us; on config 5, whose fronts are
     // thousands of cells long, 89.6 / 85.0 / 64.2 ms: the wide families pay off on large lattices only)
@@ -1350,7 +1376,8 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     if (spill_per_list_set * spill_sets >= ((size_t)1 << 32)) return FIRE_EINVAL;   // spill slots are addressed by 32-bit word offsets
     const size_t nw = (size_t)L->H * L->Ww;
     const size_t nt = (size_t)L->Tw * L->Th;
-    const size_t rescue_bytes = nw * 4 * (bt ? (size_t)L->burn_kmax + 1 : 2) * kRescueCtas;
+    const int kmax = L->burn_kmax > 1 ? L->burn_kmax : 1;
+    const size_t rescue_bytes = nw * 4 * (bt ? (size_t)kmax + 1 : 2) * kRescueCtas;
     if (nt * (size_t)S * planes >= ((size_t)1 << 31)) return FIRE_EINVAL;   // planes are addressed by 32-bit tile offsets: split the batch
     const size_t tiles_bytes = nt * 8 * (size_t)S * planes;
     if (L->status_capacity < (size_t)2 * S || L->spill_capacity < spill_bytes || L->rescue_capacity < rescue_bytes ||
@@ -1388,7 +1415,18 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     prm.work_counter = L->work_counter; prm.rescue_list = L->status; prm.spill = L->spill;
     prm.S = S; prm.P = L->P; prm.W = L->W; prm.H = L->H; prm.Ww = L->Ww; prm.Tw = L->Tw; prm.Th = L->Th; prm.num_sms = L->num_sms;
     prm.max_steps = max_steps;
-    prm.ktime = bt ? L->ktime : nullptr; prm.gt_planes = bt ? L->gt_planes : nullptr; prm.kmax = bt ? L->burn_kmax : 1;
+    if (bt && (L->ktime == nullptr || L->burn_kmax <= 1)) {               // ignition times without burn times: every cell burns one step
+        if (L->ktime == nullptr) {
+            FIRE_CUDA_TRY(L, cudaStreamSynchronize(st));
+            size_t cap = 0;
+            int rc = fire_reserve(L, (void**)&L->ktime, &cap, L->cells);
+            if (rc != FIRE_OK) return rc;
+        }
+        FIRE_CUDA_TRY(L, cudaMemsetAsync(L->ktime, 0, L->cells, st));
+    }
+    prm.ktime = bt ? L->ktime : nullptr; prm.gt_planes = bt ? L->gt_planes : nullptr; prm.kmax = kmax;
+    prm.out_time = L->out_time;
+    if (L->out_time) FIRE_CUDA_TRY(L, cudaMemsetAsync(L->out_time, 0xFF, (size_t)S * L->cells * sizeof(int32_t), st));      // -1 = never ignited
 
     // ---- launch order: largest expected fires first (only matters when there are more simulations than resident ones)
     prm.order = nullptr;

@@ -21,7 +21,7 @@ FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
     "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
-    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_landscape_set_elevation", "fire_burn_count", "fire_error_string",
+    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_set_time_output", "fire_landscape_set_elevation", "fire_burn_count", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
 
@@ -61,6 +61,7 @@ def load() -> C.CDLL:
     lib.fire_set_schedule.argtypes = [_vp, C.c_int32]
     lib.fire_set_kernel.argtypes = [_vp, C.c_int32]
     lib.fire_set_burn_time.argtypes = [_vp, _vp, C.c_int32, _vp]
+    lib.fire_set_time_output.argtypes = [_vp, _vp]
     lib.fire_landscape_set_elevation.argtypes = [_vp, _vp, _vp]
     lib.fire_burn_count.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     lib.fire_set_profiling.argtypes = [_vp, C.c_int32]
@@ -256,6 +257,16 @@ def fire_set_burn_time(L: Landscape, burn_time, stream=None) -> None:
     import numpy as np
     bt = np.ascontiguousarray(np.asarray(burn_time if burn_time is not None else [], dtype=np.uint8))
     _check(load().fire_set_burn_time(L.handle, bt.ctypes.data if bt.size else None, int(bt.size), _stream(stream)), "fire_set_burn_time")
+
+
+def fire_set_time_output(L: Landscape, out_time: torch.Tensor | None) -> None:
+    """out_time: int32 CUDA tensor [S_max][H][W] kept alive by the caller, or None to switch the output off."""
+    ptr = None
+    if out_time is not None:
+        if out_time.dtype != torch.int32 or not out_time.is_cuda or not out_time.is_contiguous() or tuple(out_time.shape[1:]) != (L.H, L.W):
+            raise TypeError("out_time must be a contiguous int32 CUDA tensor of shape [S][H][W]")
+        ptr = out_time.data_ptr()
+    _check(load().fire_set_time_output(L.handle, ptr), "fire_set_time_output")
 
 
 def fire_set_kernel(L: Landscape, family: int = 0) -> None:

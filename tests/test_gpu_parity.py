@@ -680,6 +680,45 @@ def test_dem_uphill_variant_and_hazard_map(orc, request):
     report(request, one_count_differences=n_diff)
 
 
+def test_time_of_burn_output(orc, request):
+    """the step at which every cell ignites (fire_set_time_output) against the oracle's out_time (pinned on the CPU by
+    BFS depth), with and without burn-out times, through the list spill and the rescue kernel; switching it off restores the
+    default path."""
+    rng = np.random.default_rng(91)
+    n = 0
+    for it in range(16):
+        H, W = int(rng.integers(2, 90)), int(rng.integers(2, 120))
+        ls = small_landscape(rng, H, W, nonburn=0.15)
+        S = int(rng.integers(1, 12))
+        betas = np.array([[rng.uniform(-2.0, 0.5), -0.4, 0.2, 0.9, 0.6]], np.float32)
+        ign = np.stack([rng.integers(0, W, S), rng.integers(0, H, S)], 1).astype(np.int32)
+        seeds = rng.integers(0, 2 ** 63, S).astype(np.uint64)
+        bt = [1, 1, 1, 1] if it % 2 == 0 else [1] + [int(v) for v in rng.integers(1, 5, 3)]
+        max_steps = int(rng.choice([0, 0, 9]))
+        Lo = orc_landscape(orc, ls); L = gh.make_landscape(ls)
+        gh.upload(L, betas)
+        tab = gh.thresholds(L, 0)
+        lf.fire_set_launch_geometry(L, int(rng.choice([64, 256, 1024])), 1)
+        lf.fire_set_list_capacity(L, int(rng.choice([0, 2, 16])), int(rng.choice([0, 0, 3])))
+        lf.fire_set_burn_time(L, bt)
+        times = torch.full((S, H, W), 12345, dtype=torch.int32, device="cuda")
+        lf.fire_set_time_output(L, times)
+        g = gh.simulate(L, ign, np.zeros(S, np.int32), seeds, max_steps=max_steps)
+        tg = times.cpu().numpy()
+        for s_ in range(S):
+            o = orc.simulate_burn_time(Lo, betas[0], bt, ign[s_], int(seeds[s_]), sim=s_, max_steps=max_steps, table=tab, want_time=True)
+            assert (g["burned"][s_] == o["burned"]).all() and g["steps"][s_] == o["steps"], (it, s_)
+            assert (tg[s_] == o["time"]).all(), (it, s_, np.argwhere(tg[s_] != o["time"])[:5])
+        lf.fire_set_time_output(L, None)
+        lf.fire_set_burn_time(L, None)
+        g0 = gh.simulate(L, ign, np.zeros(S, np.int32), seeds, max_steps=max_steps)
+        o0 = orc.simulate_batch(Lo, betas, ign, np.zeros(S, np.int32), seeds, max_steps=max_steps, tables=[tab])
+        assert (g0["burned"] == o0["burned"]).all() and (g0["steps"] == o0["steps"]).all()
+        n += 1
+        L.close()
+    report(request, cases=n)
+
+
 # ---------------------------------------------------------------------------------- randomised parity
 def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
     """Seeded fuzz: random lattice sizes (1 x 1 .. 140 x 200, ragged), vegetation, parameters, ignitions (some off the lattice
