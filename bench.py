@@ -48,8 +48,8 @@ UNIT = "trials/s"
 # ncu --set full capture of the propagation kernel on the workload below: dram__bytes_read.sum + dram__bytes_write.sum per
 # launch, with the commit the captured kernel was built from (profiles/README.md names the file and the command).  Refresh
 # the number together with every change of the propagation kernel; None until a capture exists for that config.
-NCU_TRAFFIC_BYTES = {3: 17482102000 + 204184320}      # profiles/r2_base_propagate_ncu.md, kernel as of commit b2a319d
-NCU_TRAFFIC_SOURCE = {3: "profiles/r2_base_propagate_ncu.md (ncu --set full, kernel of commit b2a319d)"}
+NCU_TRAFFIC_BYTES = {3: 17508026000 + 205499000}      # profiles/r2_propagate_ncu.md: capture of commit 9c53f0e (same SASS since b2a319d)
+NCU_TRAFFIC_SOURCE = {3: "profiles/r2_propagate_ncu.md (ncu --set full; two-phase kernel unchanged since commit b2a319d)"}
 
 
 def log(*a):
@@ -104,7 +104,9 @@ def run_reference(args) -> None:
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w, idx = oracle_sample(args.cfg, sample_budget(args.cfg))
+    # the whole run (warm-up + K steps) should end within a few minutes: the per-step sample shrinks with K
+    budget = sample_budget(args.cfg)
+    w, idx = oracle_sample(args.cfg, max(budget // 16, min(budget, budget * 5 // max(args.steps, 1))))
     n = len(idx)
     for _ in range(min(args.warmup, 1)):                 # the oracle has no caches to warm beyond page-in
         time_oracle(w, idx[:: 16])

@@ -96,6 +96,12 @@ int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, const int32
  * of the default local-plane test on the aspect (R-7).  Invalidates the threshold table: call fire_params_upload again. */
 int fire_landscape_set_elevation(fire_landscape* L, const float* elevation, void* stream);
 
+/* Per-class vegetation term: Eq. 1 has one vegetation term, beta_1 I_f with I_f = 1 for forest.
+ * class_if_host f32[n_classes] (HOST memory, read before the call returns) gives every vegetation class v its own I_f
+ * (classes >= n_classes get 0; class 0 cannot burn anyway); n_classes = 0 restores the paper's indicator (class 1 only).
+ * Invalidates the threshold table: call fire_params_upload again. */
+int fire_landscape_set_class_indicator(fire_landscape* L, const float* class_if_host, int32_t n_classes, void* stream);
+
 /* Hazard map: out_count u32[H][W] = number of the S maps burned u32[S][H][ceil(W/32)] in which the
  * cell is burnt (divide by S for the burn probability of the cell over replicates). */
 int fire_burn_count(fire_landscape* L, const uint32_t* burned, int32_t S, uint32_t* out_count, void* stream);

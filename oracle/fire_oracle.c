@@ -204,6 +204,30 @@ void orc_threshold_table_dem(const float beta[5], const uint8_t* veg, const floa
         }
 }
 
+/* Variant of C-2 / C-3 ("per-class I_f table"): Eq. 1 has ONE vegetation term, beta_1 I_f with I_f = 1 for forest
+ * (PAPER.md:76, :81); with more fuel classes than the paper's two (BASELINE configs have 4 and 6) a table gives every class v its
+ * own value I_f = class_if[v] (double of the f32 given).  class_if = {0, 1, 0, 0, ...} is orc_threshold_table. */
+void orc_threshold_table_classes(const float beta[5], const uint8_t* veg, const float* slope, const float* aspect,
+                                 const float* wind, const float class_if[256], int W, int H, uint32_t* out)
+{
+    double b0 = (double)beta[0], b1 = (double)beta[1], b2 = (double)beta[2], b3 = (double)beta[3], b4 = (double)beta[4];
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            size_t c = (size_t)y * W + x;
+            orc_cov cv;
+            orc_covariates(veg[c], slope[c], aspect[c], wind[c], &cv);
+            for (int d = 0; d < 8; ++d) {
+                double xx = b0 + b1 * (double)class_if[veg[c]];
+                xx = xx + b2 * cv.psi;
+                xx = xx + b3 * cv.omega[d];
+                xx = xx + b4 * cv.sigma[d];
+                double p = 1.0 / (1.0 + exp(-xx));
+                long long t = llrint(ldexp(p, 32));
+                out[c * 8 + d] = cv.burnable ? (uint32_t)(t > 0xFFFFFFFFll ? 0xFFFFFFFFll : t) : 0u;
+            }
+        }
+}
+
 /* ------------------------------------------------------------------------- *
  * C-4: one simulation (PAPER.md:91 states; :97 ignition; :99, :133 synchronous
  * update, independent trial per burning neighbour = 1 - prod(1 - p_i) in law,

@@ -75,6 +75,8 @@ def _declare(l):
     l.orc_threshold_table.restype = None
     l.orc_threshold_table_dem.argtypes = [_f32p, _u8p, _f32p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _u32p]
     l.orc_threshold_table_dem.restype = None
+    l.orc_threshold_table_classes.argtypes = [_f32p, _u8p, _f32p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _u32p]
+    l.orc_threshold_table_classes.restype = None
     l.orc_simulate.argtypes = [_u8p, _f32p, _f32p, _f32p, C.c_int, C.c_int, _f32p, _u32p,
                                C.c_int, C.c_int, C.c_uint64, C.c_uint32, C.c_uint32,
                                _u32p, _i32p, _u32p, _u64p]
@@ -182,6 +184,16 @@ def threshold_table_dem(L: Landscape, beta, elevation) -> np.ndarray:
     assert z.shape == (L.H, L.W)
     out = np.zeros((L.H, L.W, 8), np.uint32)
     lib().orc_threshold_table_dem(_p(b, _f32p), *L._ptrs(), _p(z, _f32p), L.W, L.H, _p(out, _u32p))
+    return out
+
+
+def threshold_table_classes(L: Landscape, beta, class_if) -> np.ndarray:
+    """Table with a per-class vegetation term (variant f4): class_if[v] = I_f of vegetation class v."""
+    b = _c(beta, np.float32)
+    w = np.zeros(256, np.float32)
+    w[: len(class_if)] = np.asarray(class_if, np.float32)
+    out = np.zeros((L.H, L.W, 8), np.uint32)
+    lib().orc_threshold_table_classes(_p(b, _f32p), *L._ptrs(), _p(w, _f32p), L.W, L.H, _p(out, _u32p))
     return out
 
 

@@ -23,6 +23,7 @@ struct fire_landscape {
     double*   tan_slope;     // [cells]
     double*   omega;         // [8][cells]  cos(wind - phi_d)
     uint32_t* burnable;      // [H][Ww] bitmap
+    double*   if_cell;       // [cells] I_f of the cell's class (fire_landscape_set_class_indicator), or null = forest bit of `flags`
 
     // a2: thresholds, [P][cells][8] u32, SOURCE-indexed: thr[p][b][d] = T(target b + offset(d), direction d);
     // one 32 B DRAM sector holds the 8 outgoing trials of a burning cell b

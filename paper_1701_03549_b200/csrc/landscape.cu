@@ -195,7 +195,8 @@ __global__ void __launch_bounds__(kThrTX * kThrTY, 4)
 fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int tiles_x,
                        const uint8_t* __restrict__ flags, const uint8_t* __restrict__ uphill,
                        const double* __restrict__ psi, const double* __restrict__ tan_slope,
-                       const double* __restrict__ omega, uint32_t* __restrict__ thr, float* __restrict__ param_mean)
+                       const double* __restrict__ omega, const double* __restrict__ if_cell, uint32_t* __restrict__ thr,
+                       float* __restrict__ param_mean)
 {
     __shared__ double sb[FIRE_THR_PGROUP][5];
     __shared__ double s_exp2[64];
@@ -219,7 +220,7 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
 #pragma unroll
     for (int d = 0; d < 8; ++d) om[d] = 0.0;
     if (live) {
-        If = (f & 2u) ? 1.0 : 0.0;
+        If = if_cell ? if_cell[c] : ((f & 2u) ? 1.0 : 0.0);           // per-class table (fire_landscape_set_class_indicator) or forest bit
         ps = psi[c]; ts = tan_slope[c]; up = uphill[c];
 #pragma unroll
         for (int d = 0; d < 8; ++d) om[d] = omega[(size_t)d * cells + c];
@@ -297,7 +298,8 @@ __global__ void __launch_bounds__(256)
 fire_thresholds_gather_kernel(const float* __restrict__ beta5, int W, int H,
                               const uint8_t* __restrict__ flags, const uint8_t* __restrict__ uphill,
                               const double* __restrict__ psi, const double* __restrict__ tan_slope,
-                              const double* __restrict__ omega, const uint32_t* __restrict__ thr_p, uint32_t* __restrict__ out)
+                              const double* __restrict__ omega, const double* __restrict__ if_cell, const uint32_t* __restrict__ thr_p,
+                              uint32_t* __restrict__ out)
 {
     const size_t cells = (size_t)W * H;
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // one thread per (cell, d)
@@ -313,7 +315,7 @@ fire_thresholds_gather_kernel(const float* __restrict__ beta5, int W, int H,
         T = 0u;
         if (f & 1u)
             T = fire_threshold((double)beta5[0], (double)beta5[1], (double)beta5[2], (double)beta5[3], (double)beta5[4],
-                               (f & 2u) ? 1.0 : 0.0, psi[c], omega[(size_t)d * cells + c], ((uphill[c] >> d) & 1u) ? tan_slope[c] : 0.0, kExp2Table);
+                               if_cell ? if_cell[c] : ((f & 2u) ? 1.0 : 0.0), psi[c], omega[(size_t)d * cells + c], ((uphill[c] >> d) & 1u) ? tan_slope[c] : 0.0, kExp2Table);
     }
     out[i] = T;
 }
@@ -339,7 +341,41 @@ fire_uphill_from_dem_kernel(const float* __restrict__ elevation, const double* _
     uphill[c] = (uint8_t)up;
 }
 
+struct class_table { float w[256]; };
+__global__ void __launch_bounds__(256)
+fire_class_indicator_kernel(const uint8_t* __restrict__ veg, const class_table tab, size_t cells, double* __restrict__ if_cell)
+{
+    const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < cells) if_cell[c] = (double)tab.w[veg[c]];
+}
+
 }  // namespace
+
+extern "C" int fire_landscape_set_class_indicator(fire_landscape* L, const float* class_if_host, int32_t n_classes, void* stream)
+{
+    if (L == nullptr || n_classes < 0 || n_classes > 256 || (n_classes > 0 && class_if_host == nullptr)) return FIRE_EINVAL;
+    if (L->sticky) return L->sticky;
+    fire_device_guard g(L->device);
+    if (!g.ok) return FIRE_ECUDA;
+    cudaStream_t st = (cudaStream_t)stream;
+    L->P = 0;                                                              // any table built before is stale
+    if (n_classes == 0) {                                                  // back to the paper's indicator: forest (class 1) only
+        FIRE_CUDA_TRY(L, cudaStreamSynchronize(st));
+        if (L->if_cell) { cudaFree(L->if_cell); L->if_cell = nullptr; }
+        return FIRE_OK;
+    }
+    class_table tab;
+    for (int v = 0; v < 256; ++v) tab.w[v] = v < n_classes ? class_if_host[v] : 0.0f;
+    if (L->if_cell == nullptr) {
+        size_t cap = 0;
+        int rc = fire_reserve(L, (void**)&L->if_cell, &cap, L->cells * sizeof(double));
+        if (rc != FIRE_OK) return rc;
+    }
+    fire_class_indicator_kernel<<<(unsigned)((L->cells + 255) / 256), 256, 0, st>>>(L->veg_class, tab, L->cells, L->if_cell);
+    FIRE_CUDA_TRY(L, cudaGetLastError());
+    L->launches += 1;
+    return FIRE_OK;
+}
 
 extern "C" int fire_landscape_set_elevation(fire_landscape* L, const float* elevation, void* stream)
 {
@@ -363,7 +399,7 @@ extern "C" int fire_landscape_destroy(fire_landscape* L)
         cudaDeviceSynchronize();
         void* ptrs[] = { L->flags, L->uphill, L->psi, L->tan_slope, L->omega, L->burnable, L->thr, L->beta_dev,
                          L->work_counter, L->status, L->spill, L->rescue_planes, L->ref_area, L->counts_scratch,
-                         L->burnable_tiles, L->tiles, L->order, L->param_mean, L->veg_class, L->ktime, L->gt_planes,
+                         L->burnable_tiles, L->tiles, L->order, L->param_mean, L->veg_class, L->ktime, L->gt_planes, L->if_cell,
                          L->gen_buf };
         for (void* p : ptrs) if (p) cudaFree(p);
         if (L->prof_ev[0]) for (int i = 0; i < 2 * 64; ++i) if (L->prof_ev[i]) cudaEventDestroy(L->prof_ev[i]);
@@ -443,7 +479,7 @@ extern "C" int fire_params_upload(fire_landscape* L, const float* beta, int32_t 
     const int tiles_x = (L->W + kThrTX - 1) / kThrTX, tiles_y = (L->H + kThrTY - 1) / kThrTY;
     dim3 grid((unsigned)(tiles_x * tiles_y), (unsigned)((P + FIRE_THR_PGROUP - 1) / FIRE_THR_PGROUP));
     fire_thresholds_kernel<<<grid, kThrTX * kThrTY, 0, (cudaStream_t)stream>>>(L->beta_dev, P, L->W, L->H, tiles_x, L->flags,
-                                                                                L->uphill, L->psi, L->tan_slope, L->omega, L->thr, L->param_mean);
+                                                                                L->uphill, L->psi, L->tan_slope, L->omega, L->if_cell, L->thr, L->param_mean);
     L->launches += 1;
     FIRE_CUDA_TRY(L, cudaGetLastError());
     L->P = P;
@@ -459,7 +495,7 @@ extern "C" int fire_thresholds_download(fire_landscape* L, int32_t p, uint32_t* 
     if (!g.ok) return FIRE_ECUDA;
     const size_t n = L->cells * 8;
     fire_thresholds_gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
-        L->beta_dev + (size_t)p * 5, L->W, L->H, L->flags, L->uphill, L->psi, L->tan_slope, L->omega,
+        L->beta_dev + (size_t)p * 5, L->W, L->H, L->flags, L->uphill, L->psi, L->tan_slope, L->omega, L->if_cell,
         L->thr + (size_t)p * L->cells * 8, out);
     L->launches += 1;
     FIRE_CUDA_TRY(L, cudaGetLastError());

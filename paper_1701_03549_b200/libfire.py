@@ -21,7 +21,7 @@ FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
     "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
-    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_set_time_output", "fire_landscape_set_elevation", "fire_burn_count", "fire_error_string",
+    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_set_time_output", "fire_landscape_set_elevation", "fire_landscape_set_class_indicator", "fire_burn_count", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
 
@@ -63,6 +63,7 @@ def load() -> C.CDLL:
     lib.fire_set_burn_time.argtypes = [_vp, _vp, C.c_int32, _vp]
     lib.fire_set_time_output.argtypes = [_vp, _vp]
     lib.fire_landscape_set_elevation.argtypes = [_vp, _vp, _vp]
+    lib.fire_landscape_set_class_indicator.argtypes = [_vp, _vp, C.c_int32, _vp]
     lib.fire_burn_count.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
     lib.fire_set_profiling.argtypes = [_vp, C.c_int32]
     lib.fire_profile_read.argtypes = [_vp, C.POINTER(C.c_float), C.c_int32, C.POINTER(C.c_int32)]
@@ -244,6 +245,14 @@ def fire_set_schedule(L: Landscape, mode: int = 0) -> None:
 def fire_landscape_set_elevation(L: Landscape, elevation: torch.Tensor, stream=None) -> None:
     _check(load().fire_landscape_set_elevation(L.handle, _dev(elevation, torch.float32, "elevation", (L.H, L.W)), _stream(stream)),
            "fire_landscape_set_elevation")
+
+
+def fire_landscape_set_class_indicator(L: Landscape, class_if, stream=None) -> None:
+    """class_if: sequence of I_f values per vegetation class, or None / empty for the paper's forest indicator."""
+    import numpy as np
+    w = np.ascontiguousarray(np.asarray(class_if if class_if is not None else [], dtype=np.float32))
+    _check(load().fire_landscape_set_class_indicator(L.handle, w.ctypes.data if w.size else None, int(w.size), _stream(stream)),
+           "fire_landscape_set_class_indicator")
 
 
 def fire_burn_count(L: Landscape, burned: torch.Tensor, out_count: torch.Tensor, stream=None) -> None:

@@ -24,7 +24,8 @@ typedef int (*burn_fn)(fire_landscape*, const uint8_t*, int32_t, void*);
 typedef int (*elev_fn)(fire_landscape*, const float*, void*);
 typedef int (*hazard_fn)(fire_landscape*, const uint32_t*, int32_t, uint32_t*, void*);
 typedef int (*timeout_fn)(fire_landscape*, int32_t*);
-any_fn fire_abi_table[20];
+typedef int (*classif_fn)(fire_landscape*, const float*, int32_t, void*);
+any_fn fire_abi_table[21];
 
 void fire_abi_fill(void)
 {
@@ -40,6 +41,8 @@ void fire_abi_fill(void)
     elev_fn f17 = fire_landscape_set_elevation;
     hazard_fn f18 = fire_burn_count;
     timeout_fn f19 = fire_set_time_output;
+    classif_fn f20 = fire_landscape_set_class_indicator;
+    fire_abi_table[20] = (any_fn)f20;
     fire_abi_table[19] = (any_fn)f19;
     fire_abi_table[16] = (any_fn)f16; fire_abi_table[17] = (any_fn)f17; fire_abi_table[18] = (any_fn)f18;
     fire_abi_table[0] = (any_fn)f0;   fire_abi_table[1] = (any_fn)f1;

@@ -62,3 +62,26 @@ def test_burn_count_is_the_per_cell_sum(orc):
             for x in range(W):
                 want[y, x] += int(masks[s, y, x])
     assert (got == want).all() and got.dtype == np.uint32
+
+
+def test_class_indicator_table(orc):
+    """Per-class vegetation term: the paper's indicator is the table (0, 1, 0, 0, ...); a zero table is beta_1 = 0; a table that is c
+    on every burnable class shifts beta_0 by c beta_1 (when that sum is exact in double)."""
+    rng = np.random.default_rng(6)
+    H, W = 11, 13
+    ls = {"veg": rng.integers(0, 5, (H, W)).astype(np.uint8), "slope": rng.uniform(0, 0.5, (H, W)).astype(np.float32),
+          "aspect": rng.uniform(0, 6.28, (H, W)).astype(np.float32), "wind": rng.uniform(0, 6.28, (H, W)).astype(np.float32)}
+    L = orc.Landscape(ls["veg"], ls["slope"], ls["aspect"], ls["wind"])
+    beta = np.array([-0.75, -0.5, 0.2, 0.6, 0.4], np.float32)
+    assert (orc.threshold_table_classes(L, beta, [0, 1, 0, 0, 0]) == orc.threshold_table(L, beta)).all()
+    b_no = beta.copy(); b_no[1] = 0
+    assert (orc.threshold_table_classes(L, beta, [0, 0, 0, 0, 0]) == orc.threshold_table(L, b_no)).all()
+    b_shift = b_no.copy(); b_shift[0] = np.float32(-0.75 + 2.0 * -0.5)             # exact: -1.75
+    assert (orc.threshold_table_classes(L, beta, [0, 2, 2, 2, 2]) == orc.threshold_table(L, b_shift)).all()
+    t = orc.threshold_table_classes(L, beta, [0, 1, 0.5, 0.25, 0])
+    base = orc.threshold_table(L, b_no)
+    for v, sign in [(1, -1), (2, -1), (3, -1), (4, 0)]:                          # beta_1 < 0: a positive I_f lowers the probability
+        sel = ls["veg"] == v
+        if sel.any():
+            assert ((t[sel] < base[sel]).all() if sign < 0 else (t[sel] == base[sel]).all()), v
+    assert (t[ls["veg"] == 0] == 0).all()
