@@ -190,6 +190,8 @@ def run_ours(args) -> None:
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.backend != "nccl":
+        local = local % max(torch.cuda.device_count(), 1)
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: libfire has no CPU fallback")
     torch.cuda.set_device(local)
@@ -197,7 +199,10 @@ def run_ours(args) -> None:
         # NCCL's own account of the communicator (ranks, transports, NVLS) goes to stderr: stdout carries the one JSON line
         os.environ.setdefault("NCCL_DEBUG", "INFO")
         os.environ.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:                                            # dry run of the N > 1 logic where there are fewer GPUs than ranks
+            dist.init_process_group(args.backend)
     if rank == 0:
         fire_build.build()
     if world > 1:
@@ -241,7 +246,11 @@ def run_ours(args) -> None:
         if rank == 0:
             assert (seeds_np == w.seeds).all()
     S_all, S = S, int(len(l_index))                      # S = sims of this rank from here on
-    S_pad = (S_all + world - 1) // world if strong else S          # all_gather needs equal shards
+    S_pad = S                                            # all_gather needs equal shards: the largest shard of any rank
+    if world > 1:
+        t_pad = torch.tensor([S], dtype=torch.int64, device="cuda")
+        dist.all_reduce(t_pad, op=dist.ReduceOp.MAX)
+        S_pad = int(t_pad.item())
 
     L = lf.fire_landscape_create(dev(ls["veg"]), dev(ls["slope"]), dev(ls["aspect"]), dev(ls["wind"]))
     H, Ww = L.H, L.Ww
@@ -477,6 +486,8 @@ def main() -> None:
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one generation of S sims per GPU (default); strong = ONE generation partitioned by parameter vector")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="torch.distributed backend; gloo only to dry-run the N > 1 logic with ranks sharing a GPU (timings then mean nothing)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
