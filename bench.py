@@ -24,6 +24,8 @@ N > 1   : simulations are independent -> every rank runs it
           --scaling strong: ONE generation partitioned by parameter vector: rank r uploads only its P / N
           vectors, so it builds P / N of the threshold table, and simulates their sims with batch positions as sim ids.
 
+--backend gloo : dry run of the N > 1 logic with ranks sharing one GPU (timings then mean nothing).
+
 --impl reference : this tier has no reference implementation; that arm times the CPU oracle (oracle/) as it
 stands, on a bounded sample of the same workload, on the host cores (rank 0 only).
 """
