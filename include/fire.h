@@ -112,6 +112,13 @@ int fire_burn_count(fire_landscape* L, const uint32_t* burned, int32_t S, uint32
  * NULL switches the output off (default). */
 int fire_set_time_output(fire_landscape* L, int32_t* out_time);
 
+/* Fused fitness counts (Eq. 2): every later fire_simulate_batch on this handle also writes
+ * out_counts u32[S][2] = (I, N*) against reference u32[H][ceil(W/32)], the values fire_fitness's out_counts would hold, while
+ * it converts the state planes to burnt maps (one pass over the maps saved; out_burned is still written).  Both arrays are the
+ * caller's (device), out_counts sized for the largest batch it will pass; both NULL switch the output off (default); one NULL and
+ * one not is FIRE_EINVAL. */
+int fire_set_fused_counts(fire_landscape* L, const uint32_t* reference, uint32_t* out_counts);
+
 /* Fuel-dependent burn-out time ("a burnt cell gets inactive after a given time that depends on the
  * vegetation type", :145, :68, :273; reading R-21).  burn_time_host u8[n_classes] (HOST memory, read before the call
  * returns): steps a cell of vegetation class v stays ACTIVE once ignited, 1..8 (0 reads as 1; classes >= n_classes burn one

@@ -57,6 +57,8 @@ struct fire_landscape {
     size_t    gt_capacity;
     int       burn_kmax;          // largest burn time set; <= 1 = the base model (every cell burns one step)
     int32_t*  out_time;           // fire_set_time_output: the caller's [S][H][W] ignition-time array, or null
+    const uint32_t* fit_ref;      // fire_set_fused_counts: the caller's reference bitmap and [S][2] counts, or null
+    uint32_t* fit_counts;
 
     // a7: fitness scratch
     uint32_t* ref_area;           // [1]

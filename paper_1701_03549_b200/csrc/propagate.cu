@@ -55,6 +55,8 @@ struct prop_params {
     const uint32_t* gt_planes;    // [kmax - 1][H][Ww] bit set iff the cell's burn time > j + 1 (rescue kernel), or null
     int kmax;                     // largest burn time (1 = every cell burns for one step)
     int32_t* out_time;            // [S][H][W] step at which every cell ignited (fire_set_time_output), or null
+    const uint32_t* fit_ref;      // fire_set_fused_counts: reference bitmap [H][Ww], or null
+    uint32_t* fit_counts;         // [S][2] = (I, N*) of Eq. 2, written by the finish kernel (rescued simulations: by the rescue kernel)
 };
 
 __device__ __forceinline__ uint32_t lanemask_lt()
@@ -906,27 +908,41 @@ fire_init_tiles_kernel(const uint64_t* __restrict__ burnable_tiles, uint64_t* __
 // one thread per (tile row, bitmap word column): 4 tiles in (32 B), 8 words out (one per lattice row)
 __global__ void __launch_bounds__(256)
 fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __restrict__ tiles, const uint32_t* __restrict__ plane_sel,
-                   int planes, uint32_t* __restrict__ out_burned, int H, int Ww, int Tw, int Th, int S)
+                   int planes, uint32_t* __restrict__ out_burned, int H, int Ww, int Tw, int Th, int S,
+                   const uint32_t* __restrict__ fit_ref, uint32_t* __restrict__ fit_counts)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= Th * Ww) return;
-    const int ty = i / Ww, wx = i % Ww;
+    const bool live = i < Th * Ww;                                     // no early return: the fused counts are reduced per warp
+    const int ty = live ? i / Ww : 0, wx = live ? i % Ww : 0;
     for (int s = blockIdx.y; s < S; s += gridDim.y) {                  // gridDim.y <= 65535 whatever the batch size
-        const size_t plane = (size_t)s * planes + (planes > 1 ? (plane_sel[s] & 1u) : 0u);
-        const uint64_t* const row = tiles + plane * Tw * Th + (size_t)ty * Tw;
-        uint64_t tl[4];
+        uint32_t n_both = 0u, n_burnt = 0u;
+        if (live) {
+            const size_t plane = (size_t)s * planes + (planes > 1 ? (plane_sel[s] & 1u) : 0u);
+            const uint64_t* const row = tiles + plane * Tw * Th + (size_t)ty * Tw;
+            uint64_t tl[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) tl[k] = (4 * wx + k < Tw) ? __ldcs(reinterpret_cast<const unsigned long long*>(row + 4 * wx + k)) : 0ull;
-        uint32_t* const out = out_burned + (size_t)s * H * Ww;
+            for (int k = 0; k < 4; ++k) tl[k] = (4 * wx + k < Tw) ? __ldcs(reinterpret_cast<const unsigned long long*>(row + 4 * wx + k)) : 0ull;
+            uint32_t* const out = out_burned + (size_t)s * H * Ww;
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int y = ty * 8 + r;
-            if (y < H) {
-                uint32_t susw = 0u;
+            for (int r = 0; r < 8; ++r) {
+                const int y = ty * 8 + r;
+                if (y < H) {
+                    uint32_t susw = 0u;
 #pragma unroll
-                for (int k = 0; k < 4; ++k) susw |= (uint32_t)((tl[k] >> (8 * r)) & 0xFFull) << (8 * k);
-                const size_t wi = (size_t)y * Ww + wx;
-                out[wi] = __ldg(burnable + wi) & ~susw;
+                    for (int k = 0; k < 4; ++k) susw |= (uint32_t)((tl[k] >> (8 * r)) & 0xFFull) << (8 * k);
+                    const size_t wi = (size_t)y * Ww + wx;
+                    const uint32_t bw = __ldg(burnable + wi) & ~susw;
+                    out[wi] = bw;
+                    if (fit_counts) { n_burnt += __popc(bw); n_both += __popc(bw & __ldg(fit_ref + wi)); }
+                }
+            }
+        }
+        if (fit_counts) {                                              // Eq. 2's two counts, fused (fire_set_fused_counts)
+            n_both = __reduce_add_sync(0xFFFFFFFFu, n_both);
+            n_burnt = __reduce_add_sync(0xFFFFFFFFu, n_burnt);
+            if ((threadIdx.x & 31) == 0 && (n_both | n_burnt)) {
+                if (n_both) atomicAdd(fit_counts + 2 * (size_t)s, n_both);
+                atomicAdd(fit_counts + 2 * (size_t)s + 1, n_burnt);
             }
         }
     }
@@ -973,11 +989,32 @@ __device__ __forceinline__ uint32_t plane_word(const uint32_t* plane, int y, int
     return ((unsigned)y < (unsigned)H && (unsigned)wx < (unsigned)Ww) ? __ldcg(plane + (size_t)y * Ww + wx) : 0u;
 }
 
+// fire_set_fused_counts for a rescued simulation: the finish kernel counted the fast kernel's half-done plane, so the rescue
+// kernel OVERWRITES (I, N*) with the counts of the map it has just written.  Called by every thread of the CTA.
+__device__ __forceinline__ void rescue_fused_counts(const prop_params& prm, const uint32_t* burned, uint32_t s, unsigned int* s_fit)
+{
+    const size_t nw = (size_t)prm.H * prm.Ww;
+    if (threadIdx.x == 0) { s_fit[0] = 0u; s_fit[1] = 0u; }
+    __syncthreads();                                  // also orders the block's own writes to `burned` before the reads below
+    uint32_t n_both = 0u, n_burnt = 0u;
+    for (size_t w = threadIdx.x; w < nw; w += blockDim.x) {
+        const uint32_t bw = __ldcg(burned + w);
+        n_burnt += __popc(bw);
+        n_both += __popc(bw & __ldg(prm.fit_ref + w));
+    }
+    n_both = __reduce_add_sync(0xFFFFFFFFu, n_both);
+    n_burnt = __reduce_add_sync(0xFFFFFFFFu, n_burnt);
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&s_fit[0], n_both); atomicAdd(&s_fit[1], n_burnt); }
+    __syncthreads();
+    if (threadIdx.x == 0) { prm.fit_counts[2 * (size_t)s] = s_fit[0]; prm.fit_counts[2 * (size_t)s + 1] = s_fit[1]; }
+}
+
 __global__ void __launch_bounds__(256)
 fire_propagate_rescue_kernel(const prop_params prm, uint32_t* planes)
 {
     __shared__ int s_y0, s_y1;
     __shared__ unsigned long long s_trials;
+    __shared__ unsigned int s_fit[2];
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int W = prm.W, H = prm.H, Ww = prm.Ww;
     const size_t nw = (size_t)H * Ww;
@@ -1068,6 +1105,7 @@ fire_propagate_rescue_kernel(const prop_params prm, uint32_t* planes)
             for (size_t w = tid; w < n; w += nthr) { cur[lo + w] = 0u; nxt[lo + w] = 0u; }
         }
         if (my_trials) atomicAdd(&s_trials, my_trials);
+        if (prm.fit_counts) rescue_fused_counts(prm, burned, s, s_fit);
         __syncthreads();
         if (tid == 0) {
             if (prm.out_steps) prm.out_steps[s] = t;
@@ -1096,6 +1134,7 @@ fire_propagate_rescue_bt_kernel(const prop_params prm, uint32_t* planes)
 {
     __shared__ int s_y0, s_y1;
     __shared__ unsigned long long s_trials;
+    __shared__ unsigned int s_fit[2];
     const int tid = threadIdx.x, nthr = blockDim.x;
     const int W = prm.W, H = prm.H, Ww = prm.Ww;
     const size_t nw = (size_t)H * Ww;
@@ -1192,6 +1231,7 @@ fire_propagate_rescue_bt_kernel(const prop_params prm, uint32_t* planes)
                 for (size_t w = tid; w < n; w += nthr) ring[(size_t)r * nw + lo + w] = 0u;
         }
         if (my_trials) atomicAdd(&s_trials, my_trials);
+        if (prm.fit_counts) rescue_fused_counts(prm, burned, s, s_fit);
         __syncthreads();
         if (tid == 0) {
             if (prm.out_steps) prm.out_steps[s] = t;
@@ -1284,6 +1324,14 @@ extern "C" int fire_set_burn_time(fire_landscape* L, const uint8_t* burn_time_ho
     FIRE_CUDA_TRY(L, cudaGetLastError());
     L->launches += 1;
     L->burn_kmax = kmax;
+    return FIRE_OK;
+}
+
+extern "C" int fire_set_fused_counts(fire_landscape* L, const uint32_t* reference, uint32_t* out_counts)
+{
+    if (L == nullptr || (reference == nullptr) != (out_counts == nullptr)) return FIRE_EINVAL;      // set or cleared together
+    L->fit_ref = reference;
+    L->fit_counts = out_counts;
     return FIRE_OK;
 }
 
@@ -1426,6 +1474,9 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     }
     prm.ktime = bt ? L->ktime : nullptr; prm.gt_planes = bt ? L->gt_planes : nullptr; prm.kmax = kmax;
     prm.out_time = L->out_time;
+    prm.fit_ref = L->fit_ref;
+    prm.fit_counts = L->fit_counts;
+    if (L->fit_counts) FIRE_CUDA_TRY(L, cudaMemsetAsync(L->fit_counts, 0, (size_t)S * 2 * sizeof(uint32_t), st));
     if (L->out_time) FIRE_CUDA_TRY(L, cudaMemsetAsync(L->out_time, 0xFF, (size_t)S * L->cells * sizeof(int32_t), st));      // -1 = never ignited
 
     // ---- launch order: largest expected fires first (only matters when there are more simulations than resident ones)
@@ -1482,7 +1533,7 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     {
         const size_t n = (size_t)L->Th * L->Ww;
         fire_finish_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)(S < 65535 ? S : 65535)), 256, 0, st>>>(L->burnable, L->tiles, L->status + S, planes, out_burned,
-                                                                                          L->H, L->Ww, L->Tw, L->Th, S);
+                                                                                          L->H, L->Ww, L->Tw, L->Th, S, L->fit_ref, L->fit_counts);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
     if (bt) fire_propagate_rescue_bt_kernel<<<kRescueCtas, 256, 0, st>>>(prm, L->rescue_planes);

@@ -21,7 +21,7 @@ FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
     "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
-    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_set_time_output", "fire_landscape_set_elevation", "fire_landscape_set_class_indicator", "fire_burn_count", "fire_error_string",
+    "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_set_time_output", "fire_set_fused_counts", "fire_landscape_set_elevation", "fire_landscape_set_class_indicator", "fire_burn_count", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
 
@@ -62,6 +62,7 @@ def load() -> C.CDLL:
     lib.fire_set_kernel.argtypes = [_vp, C.c_int32]
     lib.fire_set_burn_time.argtypes = [_vp, _vp, C.c_int32, _vp]
     lib.fire_set_time_output.argtypes = [_vp, _vp]
+    lib.fire_set_fused_counts.argtypes = [_vp, _vp, _vp]
     lib.fire_landscape_set_elevation.argtypes = [_vp, _vp, _vp]
     lib.fire_landscape_set_class_indicator.argtypes = [_vp, _vp, C.c_int32, _vp]
     lib.fire_burn_count.argtypes = [_vp, _vp, C.c_int32, _vp, _vp]
@@ -276,6 +277,19 @@ def fire_set_time_output(L: Landscape, out_time: torch.Tensor | None) -> None:
             raise TypeError("out_time must be a contiguous int32 CUDA tensor of shape [S][H][W]")
         ptr = out_time.data_ptr()
     _check(load().fire_set_time_output(L.handle, ptr), "fire_set_time_output")
+
+
+def fire_set_fused_counts(L: Landscape, reference: torch.Tensor | None, out_counts: torch.Tensor | None) -> None:
+    """reference i32[H][Ww], out_counts i32[S_max][2]: CUDA tensors kept alive by the caller; both None switch the output off."""
+    if (reference is None) != (out_counts is None):
+        raise TypeError("reference and out_counts are set or cleared together")
+    rp = cp = None
+    if reference is not None:
+        rp = _dev(reference, torch.int32, "reference", (L.H, L.Ww))
+        if out_counts.dtype != torch.int32 or not out_counts.is_cuda or not out_counts.is_contiguous() or tuple(out_counts.shape[1:]) != (2,):
+            raise TypeError("out_counts must be a contiguous int32 CUDA tensor of shape [S][2]")
+        cp = out_counts.data_ptr()
+    _check(load().fire_set_fused_counts(L.handle, rp, cp), "fire_set_fused_counts")
 
 
 def fire_set_kernel(L: Landscape, family: int = 0) -> None:

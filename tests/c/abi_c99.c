@@ -24,8 +24,9 @@ typedef int (*burn_fn)(fire_landscape*, const uint8_t*, int32_t, void*);
 typedef int (*elev_fn)(fire_landscape*, const float*, void*);
 typedef int (*hazard_fn)(fire_landscape*, const uint32_t*, int32_t, uint32_t*, void*);
 typedef int (*timeout_fn)(fire_landscape*, int32_t*);
+typedef int (*fused_fn)(fire_landscape*, const uint32_t*, uint32_t*);
 typedef int (*classif_fn)(fire_landscape*, const float*, int32_t, void*);
-any_fn fire_abi_table[21];
+any_fn fire_abi_table[22];
 
 void fire_abi_fill(void)
 {
@@ -42,6 +43,8 @@ void fire_abi_fill(void)
     hazard_fn f18 = fire_burn_count;
     timeout_fn f19 = fire_set_time_output;
     classif_fn f20 = fire_landscape_set_class_indicator;
+    fused_fn f21 = fire_set_fused_counts;
+    fire_abi_table[21] = (any_fn)f21;
     fire_abi_table[20] = (any_fn)f20;
     fire_abi_table[19] = (any_fn)f19;
     fire_abi_table[16] = (any_fn)f16; fire_abi_table[17] = (any_fn)f17; fire_abi_table[18] = (any_fn)f18;

@@ -719,6 +719,52 @@ def test_time_of_burn_output(orc, request):
     report(request, cases=n)
 
 
+def test_fused_fitness_counts(orc, request):
+    """Eq. 2's counts (I, N*) written by fire_simulate_batch itself (fire_set_fused_counts) equal the oracle's counts
+    of the same maps -- on every kernel family, through the list spill, the rescue kernel (which overwrites the counts of the
+    simulations it redoes) and the burn-out variant; the maps themselves are unchanged and switching it off stops the writes."""
+    w = wl.load_workload(2)
+    ls = w.landscape
+    L = gh.make_landscape(ls)
+    gh.upload(L, w.betas)
+    Lo = orc_landscape(orc, ls)
+    ref = orc.simulate(Lo, w.ref_beta, w.ref_ignition, w.ref_seed, sim=0)["burned"]
+    base = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    oc, _, _ = orc.fitness(ref, base["burned"], Lo.W, 0)
+    ref_d = torch.from_numpy(ref.view(np.int32)).cuda()
+    n = 0
+    for threads, per_sm, shared, total, family, bt in [(0, 0, 0, 0, 0, None), (256, 4, 8, 8, 1, None), (128, 4, 1, 1, 2, None),
+                                                       (1024, 1, 0, 0, 3, None), (256, 2, 5, 4096, 4, None), (64, 3, 2, 3, 0, None),
+                                                       (0, 0, 0, 0, 0, [1, 1, 1, 1]), (256, 4, 2, 3, 0, [1, 3, 2, 4])]:
+        counts = torch.full((w.S + 3, 2), 77, dtype=torch.int32, device="cuda")
+        lf.fire_set_launch_geometry(L, threads, per_sm)
+        lf.fire_set_list_capacity(L, shared, total)
+        lf.fire_set_kernel(L, family)
+        lf.fire_set_burn_time(L, bt)
+        lf.fire_set_fused_counts(L, ref_d, counts)
+        g = gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+        got = counts.cpu().numpy().view(np.uint32)
+        if bt is None or max(bt) == 1:
+            assert (g["burned"] == base["burned"]).all()
+            want = oc
+        else:
+            want, _, _ = orc.fitness(ref, g["burned"], Lo.W, 0)
+        assert (got[: w.S] == want).all(), (threads, per_sm, shared, total, family, bt, np.flatnonzero((got[: w.S] != want).any(axis=1))[:8])
+        assert (got[w.S:] == 77).all()                                   # nothing past the batch is touched
+        c2, _, _ = gh.fitness(L, ref, g["burned"], 0)
+        assert (c2 == want).all()
+        n += 1
+    lf.fire_set_fused_counts(L, None, None)
+    lf.fire_set_burn_time(L, None)
+    counts.fill_(55)
+    gh.simulate(L, w.ignitions, w.sim_param, w.seeds)
+    assert (counts.cpu().numpy() == 55).all()
+    with pytest.raises(TypeError):
+        lf.fire_set_fused_counts(L, ref_d, None)
+    L.close()
+    report(request, cases=n)
+
+
 # ---------------------------------------------------------------------------------- randomised parity
 def test_random_lattices_geometries_and_kernels_match_the_oracle(orc, request):
     """Seeded fuzz: random lattice sizes (1 x 1 .. 140 x 200, ragged), vegetation, parameters, ignitions (some off the lattice
