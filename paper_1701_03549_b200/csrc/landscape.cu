@@ -105,38 +105,11 @@ __constant__ double kExp2Table[64] = {      // 2^(j/64), j = 0..63, correctly ro
     1.9152065613971474, 1.9360617934922943, 1.9571441241754002, 1.978456026387951
 };
 
-__device__ __forceinline__ uint32_t fire_threshold_from_x(double x, const double* __restrict__ tbl)
-{
-    // clamp to [-40, 40] with integer operations on the high word (the FP64 pipe is the bottleneck)
-    double y = -x;
-    const uint32_t yh = (uint32_t)__double2hiint(y);
-    if ((yh & 0x7FFFFFFFu) >= 0x40440000u) y = __hiloint2double((int)((yh & 0x80000000u) | 0x40440000u), 0);
-    const double t = __fma_rn(y, 92.33248261689366, 6755399441055744.0);        // 2^52 + 2^51: low word = n = rint(64 y log2 e)
-    const double nf = t - 6755399441055744.0;
-    double r = __fma_rn(nf, -0.010830424667801708, y);                            // ln 2 / 64, high part (24 trailing zero bits)
-    r = __fma_rn(nf, -2.8447437476627285e-11, r);                                 // low part
-    double q = 8.33333333333333333333e-03;                                        // 1/120
-    q = __fma_rn(q, r, 4.16666666666666666667e-02);
-    q = __fma_rn(q, r, 1.66666666666666666667e-01);
-    q = __fma_rn(q, r, 0.5);
-    q = __fma_rn(q, r, 1.0);
-    q = __fma_rn(q, r, 1.0);
-    const int n = __double2loint(t);
-    q = q * tbl[n & 63];
-    const double e = __hiloint2double(__double2hiint(q) + ((n >> 6) << 20), __double2loint(q));   // q 2^k, |k| <= 58
-    const double d = 1.0 + e;
-    double rc;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc) : "d"(d));
-    rc = __fma_rn(rc, __fma_rn(-d, rc, 1.0), rc);
-    rc = __fma_rn(rc, __fma_rn(-d, rc, 1.0), rc);
-    const double v = __fma_rn(rc, 4294967296.0, 4503599627370496.0);              // 2^52 + rint(p 2^32), 0 <= rint <= 2^32
-    const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
-    return (hi & 1u) ? 0xFFFFFFFFu : lo;                                          // min(., 2^32 - 1)
-}
-
-// The same for N independent arguments, written step by step across them so that the N dependent chains interleave in the
-// instruction stream (one chain alone waits for the latency of every operation).
-template <int N>
+// N independent arguments, written step by step across them so that the N dependent chains interleave in the instruction stream
+// (one chain alone waits for the latency of every operation).  kSafe = false leaves out the clamp and the saturation: the caller
+// guarantees |x| < 21 (no clamp needed, and rint(p 2^32) < 2^32 because p 2^32 reaches 2^32 - 0.5 at x = 22.9 only); both
+// variants run the same operations on the same values there, so they return the same bits.
+template <int N, bool kSafe>
 __device__ __forceinline__ void fire_thresholds_from_x(const double (&x)[N], const double* __restrict__ tbl, uint32_t (&T)[N])
 {
     double y[N], t[N], r[N], q[N], d[N], rc[N];
@@ -144,13 +117,20 @@ __device__ __forceinline__ void fire_thresholds_from_x(const double (&x)[N], con
 #pragma unroll
     for (int i = 0; i < N; ++i) {
         y[i] = -x[i];
-        const uint32_t yh = (uint32_t)__double2hiint(y[i]);
-        if ((yh & 0x7FFFFFFFu) >= 0x40440000u) y[i] = __hiloint2double((int)((yh & 0x80000000u) | 0x40440000u), 0);
+        if (kSafe) {      // clamp to [-40, 40] with integer operations on the high word (the FP64 pipe is the bottleneck)
+            const uint32_t yh = (uint32_t)__double2hiint(y[i]);
+            if ((yh & 0x7FFFFFFFu) >= 0x40440000u) y[i] = __hiloint2double((int)((yh & 0x80000000u) | 0x40440000u), 0);
+        }
     }
 #pragma unroll
-    for (int i = 0; i < N; ++i) t[i] = __fma_rn(y[i], 92.33248261689366, 6755399441055744.0);
+    for (int i = 0; i < N; ++i) t[i] = __fma_rn(y[i], 92.33248261689366, 6755399441055744.0);      // 2^52 + 2^51: low word = n = rint(64 y log2 e)
 #pragma unroll
-    for (int i = 0; i < N; ++i) { const double nf = t[i] - 6755399441055744.0; r[i] = __fma_rn(nf, -0.010830424667801708, y[i]); r[i] = __fma_rn(nf, -2.8447437476627285e-11, r[i]); n[i] = __double2loint(t[i]); }
+    for (int i = 0; i < N; ++i) {
+        const double nf = t[i] - 6755399441055744.0;
+        r[i] = __fma_rn(nf, -0.010830424667801708, y[i]);                  // ln 2 / 64, high part (24 trailing zero bits)
+        r[i] = __fma_rn(nf, -2.8447437476627285e-11, r[i]);                // low part
+        n[i] = __double2loint(t[i]);
+    }
 #pragma unroll
     for (int i = 0; i < N; ++i) q[i] = __fma_rn(8.33333333333333333333e-03, r[i], 4.16666666666666666667e-02);
 #pragma unroll
@@ -165,20 +145,31 @@ __device__ __forceinline__ void fire_thresholds_from_x(const double (&x)[N], con
     for (int i = 0; i < N; ++i) q[i] = q[i] * tbl[n[i] & 63];
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        const double e = __hiloint2double(__double2hiint(q[i]) + ((n[i] >> 6) << 20), __double2loint(q[i]));
+        const double e = __hiloint2double(__double2hiint(q[i]) + ((n[i] >> 6) << 20), __double2loint(q[i]));   // q 2^k, |k| <= 58
         d[i] = 1.0 + e;
         asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(rc[i]) : "d"(d[i]));
     }
+    // one cubic step from the 20-bit estimate: err = 1 - d rc, rc (1 + err + err^2) leaves err^3 = 2^-60
 #pragma unroll
-    for (int i = 0; i < N; ++i) rc[i] = __fma_rn(rc[i], __fma_rn(-d[i], rc[i], 1.0), rc[i]);
+    for (int i = 0; i < N; ++i) d[i] = __fma_rn(-d[i], rc[i], 1.0);
 #pragma unroll
-    for (int i = 0; i < N; ++i) rc[i] = __fma_rn(rc[i], __fma_rn(-d[i], rc[i], 1.0), rc[i]);
+    for (int i = 0; i < N; ++i) d[i] = __fma_rn(d[i], d[i], d[i]);
+#pragma unroll
+    for (int i = 0; i < N; ++i) rc[i] = __fma_rn(rc[i], d[i], rc[i]);
 #pragma unroll
     for (int i = 0; i < N; ++i) {
-        const double v = __fma_rn(rc[i], 4294967296.0, 4503599627370496.0);
+        const double v = __fma_rn(rc[i], 4294967296.0, 4503599627370496.0);          // 2^52 + rint(p 2^32), 0 <= rint <= 2^32
         const uint32_t lo = (uint32_t)__double2loint(v), hi = (uint32_t)__double2hiint(v);
-        T[i] = (hi & 1u) ? 0xFFFFFFFFu : lo;
+        T[i] = (kSafe && (hi & 1u)) ? 0xFFFFFFFFu : lo;                              // min(., 2^32 - 1)
     }
+}
+
+__device__ __forceinline__ uint32_t fire_threshold_from_x(double x, const double* __restrict__ tbl)
+{
+    const double x1[1] = { x };
+    uint32_t T1[1];
+    fire_thresholds_from_x<1, true>(x1, tbl, T1);
+    return T1[0];
 }
 
 // x of Eq. 1 for one (target, direction): every operation one IEEE double operation, in the order of C-3
@@ -191,6 +182,33 @@ __device__ __forceinline__ uint32_t fire_threshold(double b0, double b1, double 
 }
 
 constexpr int kThrChains = 4;      // directions evaluated side by side (4 x 2 passes; 8 at once needs 108 registers and is slower)
+
+// The 8 thresholds of one target cell into the transposition buffer; returns the sum of the 8 probabilities (scheduling hint).
+template <bool kSafe>
+__device__ __forceinline__ float fire_thresholds_of_cell(double base, double b3, double b4ts, const double (&om)[8], uint32_t up, bool live,
+                                                         const double* __restrict__ tbl, uint32_t (*sT)[kThrTY + 2][kThrTX + 2], int lx, int ly)
+{
+    float fsum = 0.0f;
+#pragma unroll
+    for (int h = 0; h < 8 / kThrChains; ++h) {
+        double x4[kThrChains];
+        uint32_t T4[kThrChains];
+#pragma unroll
+        for (int i = 0; i < kThrChains; ++i) {
+            const int d = kThrChains * h + i;
+            x4[i] = __dadd_rn(__dadd_rn(base, __dmul_rn(b3, om[d])), ((up >> d) & 1u) ? b4ts : 0.0);
+        }
+        fire_thresholds_from_x<kThrChains, kSafe>(x4, tbl, T4);
+#pragma unroll
+        for (int i = 0; i < kThrChains; ++i) {
+            const int d = kThrChains * h + i;
+            const uint32_t T = live ? T4[i] : 0u;
+            sT[d][ly - fire_dy(d) + 1][lx - fire_dx(d) + 1] = T;      // slot d of the source = target - offset(d)
+            fsum += (float)T * 2.3283064365386963e-10f;
+        }
+    }
+    return fsum;
+}
 __global__ void __launch_bounds__(kThrTX * kThrTY, 4)
 fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int tiles_x,
                        const uint8_t* __restrict__ flags, const uint8_t* __restrict__ uphill,
@@ -199,13 +217,14 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
                        float* __restrict__ param_mean)
 {
     __shared__ double sb[FIRE_THR_PGROUP][5];
+    __shared__ float sab[FIRE_THR_PGROUP][5];                             // |beta|
     __shared__ double s_exp2[64];
     __shared__ float s_mean[FIRE_THR_PGROUP];
     __shared__ uint32_t sT2[2][8][kThrTY + 2][kThrTX + 2];                // [buffer][d][source row + 1][source column + 1]
     const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
     const int p0 = blockIdx.y * FIRE_THR_PGROUP;
     const int np = min(FIRE_THR_PGROUP, P - p0);
-    if (tid < np * 5) sb[tid / 5][tid % 5] = (double)beta[(size_t)p0 * 5 + tid];
+    if (tid < np * 5) { const float bv = beta[(size_t)p0 * 5 + tid]; sb[tid / 5][tid % 5] = (double)bv; sab[tid / 5][tid % 5] = fabsf(bv); }
     if (tid < FIRE_THR_PGROUP) s_mean[tid] = 0.0f;
     if (tid < 64) s_exp2[tid] = kExp2Table[tid];
     const int x0 = (int)(blockIdx.x % tiles_x) * kThrTX, y0 = (int)(blockIdx.x / tiles_x) * kThrTY;
@@ -225,66 +244,78 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
 #pragma unroll
         for (int d = 0; d < 8; ++d) om[d] = omega[(size_t)d * cells + c];
     }
-    // the sources this thread writes out: its own cell, and (threads 0..83) one cell of the ring around the tile
+    // largest |covariate| over the warp, in single precision (non-negative floats order like their bit patterns; a NaN wins)
+    uint32_t om_bits = 0u;
+#pragma unroll
+    for (int d = 0; d < 8; ++d) om_bits = max(om_bits, __float_as_uint(fabsf((float)om[d])));
+    const float m_om = __uint_as_float(__reduce_max_sync(0xFFFFFFFFu, om_bits));
+    const float m_if = __uint_as_float(__reduce_max_sync(0xFFFFFFFFu, __float_as_uint(fabsf((float)If))));
+    const float m_ps = __uint_as_float(__reduce_max_sync(0xFFFFFFFFu, __float_as_uint(fabsf((float)ps))));
+    const float m_ts = __uint_as_float(__reduce_max_sync(0xFFFFFFFFu, __float_as_uint(fabsf((float)ts))));
+    // the sources this thread writes out: its own cell, and (threads 0..83) one cell of the ring around the tile.  Which of
+    // their 8 slots this tile holds does not depend on the parameter vector: one bit mask each, worked out once.
     int hx = -2, hy = -2;                                                 // ring cell in tile coordinates, if any
     if (tid < 2 * kThrTX) { hx = tid & 31; hy = (tid < kThrTX) ? -1 : kThrTY; }
     else if (tid < 2 * kThrTX + 2 * kThrTY) { const int k = tid - 2 * kThrTX; hx = (k < kThrTY) ? -1 : kThrTX; hy = k % kThrTY; }
     else if (tid < 2 * kThrTX + 2 * kThrTY + 4) { const int k = tid - 2 * kThrTX - 2 * kThrTY; hx = (k & 1) ? kThrTX : -1; hy = (k & 2) ? kThrTY : -1; }
+    uint32_t own_mask = 0u, ring_mask = 0u;
+    uint32_t ring_c = 0;                                                  // the host checks W * H < 2^31
+    if (inside) {
+#pragma unroll
+        for (int d = 0; d < 8; ++d) {
+            const int tx = lx + fire_dx(d), ty = ly + fire_dy(d);
+            if (tx >= 0 && tx < kThrTX && ty >= 0 && ty < kThrTY) own_mask |= 1u << d;
+        }
+    }
+    if (hx != -2) {
+        const int gx = x0 + hx, gy = y0 + hy;
+        if (gx >= 0 && gx < W && gy >= 0 && gy < H) {
+            ring_c = (uint32_t)gy * (uint32_t)W + (uint32_t)gx;
+#pragma unroll
+            for (int d = 0; d < 8; ++d) {
+                const int tx = hx + fire_dx(d), ty = hy + fire_dy(d);
+                if (tx >= 0 && tx < kThrTX && ty >= 0 && ty < kThrTY) ring_mask |= 1u << d;
+            }
+        }
+    }
+    const int hx1 = hx + 1, hy1 = hy + 1;
     __syncthreads();
     for (int q = 0; q < np; ++q) {
         const double b0 = sb[q][0], b1 = sb[q][1], b2 = sb[q][2], b3 = sb[q][3], b4 = sb[q][4];
         uint32_t (*sT)[kThrTY + 2][kThrTX + 2] = sT2[q & 1];         // double-buffered: one barrier per parameter vector
         float fsum = 0.0f;
         // Eq. 1 for the 8 directions of this target: x in the order of C-3, one IEEE operation each; non-burnable targets run
-        // the same arithmetic on zeros and are masked at the end (no branch: the chains of 4 directions interleave)
+        // the same arithmetic on zeros and are masked at the end (no branch: the chains of 4 directions interleave).
+        // b4 sigma_d is b4 tan(slope) or b4 0 = +-0; adding +-0 changes nothing (x = +-0 gives the same threshold).
         const double base = __dadd_rn(__dadd_rn(b0, __dmul_rn(b1, If)), __dmul_rn(b2, ps));
-#pragma unroll
-        for (int h = 0; h < 8 / kThrChains; ++h) {
-            double x4[kThrChains];
-            uint32_t T4[kThrChains];
-#pragma unroll
-            for (int i = 0; i < kThrChains; ++i) {
-                const int d = kThrChains * h + i;
-                x4[i] = __dadd_rn(__dadd_rn(base, __dmul_rn(b3, om[d])), __dmul_rn(b4, ((up >> d) & 1u) ? ts : 0.0));
-            }
-            fire_thresholds_from_x<kThrChains>(x4, s_exp2, T4);
-#pragma unroll
-            for (int i = 0; i < kThrChains; ++i) {
-                const int d = kThrChains * h + i;
-                const uint32_t T = live ? T4[i] : 0u;
-                sT[d][ly - fire_dy(d) + 1][lx - fire_dx(d) + 1] = T;      // slot d of the source = target - offset(d)
-                fsum += (float)T * 2.3283064365386963e-10f;
-            }
-        }
+        const double b4ts = __dmul_rn(b4, ts);
+        // |x| <= |b0| + |b1| max|If| + |b2| max|psi| + |b3| max|omega| + |b4| max|tan| over the warp (single precision is enough
+        // for a bound): below 20, neither the clamp (|x| >= 40) nor the saturation (x >= 22.9) can act.  NaN compares false.
+        const float bound = fmaf(sab[q][4], m_ts, fmaf(sab[q][3], m_om, fmaf(sab[q][2], m_ps, fmaf(sab[q][1], m_if, sab[q][0]))));
+        const bool fast = __all_sync(0xFFFFFFFFu, bound < 20.0f);
+        if (fast) fsum = fire_thresholds_of_cell<false>(base, b3, b4ts, om, up, live, s_exp2, sT, lx, ly);
+        else fsum = fire_thresholds_of_cell<true>(base, b3, b4ts, om, up, live, s_exp2, sT, lx, ly);
         // scheduling hint only (never enters a result): sum of the contagion probabilities of this parameter vector
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) fsum += __shfl_xor_sync(0xFFFFFFFFu, fsum, o);
         if (lx == 0) atomicAdd(&s_mean[q], fsum);
         __syncthreads();
         uint32_t* const tp = thr + (size_t)(p0 + q) * cells * 8;
-        if (inside) {                                                     // own cell as a source
+        if (own_mask == 0xFFu) {                                          // own cell as a source: a whole sector
             uint32_t* const out = tp + c * 8;
-            if (lx >= 1 && lx <= kThrTX - 2 && ly >= 1 && ly <= kThrTY - 2) {
-                reinterpret_cast<uint4*>(out)[0] = make_uint4(sT[0][ly + 1][lx + 1], sT[1][ly + 1][lx + 1], sT[2][ly + 1][lx + 1], sT[3][ly + 1][lx + 1]);
-                reinterpret_cast<uint4*>(out)[1] = make_uint4(sT[4][ly + 1][lx + 1], sT[5][ly + 1][lx + 1], sT[6][ly + 1][lx + 1], sT[7][ly + 1][lx + 1]);
-            } else {
+            reinterpret_cast<uint4*>(out)[0] = make_uint4(sT[0][ly + 1][lx + 1], sT[1][ly + 1][lx + 1], sT[2][ly + 1][lx + 1], sT[3][ly + 1][lx + 1]);
+            reinterpret_cast<uint4*>(out)[1] = make_uint4(sT[4][ly + 1][lx + 1], sT[5][ly + 1][lx + 1], sT[6][ly + 1][lx + 1], sT[7][ly + 1][lx + 1]);
+        } else if (own_mask) {                                            // on the tile's edge: the slots whose targets are in the tile
+            uint32_t* const out = tp + c * 8;
 #pragma unroll
-                for (int d = 0; d < 8; ++d) {
-                    const int tx = lx + fire_dx(d), ty = ly + fire_dy(d);
-                    if (tx >= 0 && tx < kThrTX && ty >= 0 && ty < kThrTY) out[d] = sT[d][ly + 1][lx + 1];
-                }
-            }
+            for (int d = 0; d < 8; ++d)
+                if ((own_mask >> d) & 1u) out[d] = sT[d][ly + 1][lx + 1];
         }
-        if (hx != -2) {                                                   // one cell of the ring around the tile
-            const int gx = x0 + hx, gy = y0 + hy;
-            if (gx >= 0 && gx < W && gy >= 0 && gy < H) {
-                uint32_t* const out = tp + ((size_t)gy * W + gx) * 8;
+        if (ring_mask) {                                                  // one cell of the ring around the tile
+            uint32_t* const out = tp + (size_t)ring_c * 8;
 #pragma unroll
-                for (int d = 0; d < 8; ++d) {
-                    const int tx = hx + fire_dx(d), ty = hy + fire_dy(d);
-                    if (tx >= 0 && tx < kThrTX && ty >= 0 && ty < kThrTY) out[d] = sT[d][hy + 1][hx + 1];
-                }
-            }
+            for (int d = 0; d < 8; ++d)
+                if ((ring_mask >> d) & 1u) out[d] = sT[d][hy1][hx1];
         }
     }
     __syncthreads();
