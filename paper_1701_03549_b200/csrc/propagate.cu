@@ -514,7 +514,7 @@ fire_propagate_kernel(const prop_params prm)
             // ---- phase 2: one Bernoulli trial per lane-slot.  Philox4x32-10(counter = (cell, t, sim, d >> 2), key = seed),
             // word d & 3 (C-1).  Round keys are rebuilt once per step (they are dead during phase 1) and made
             // opaque so that they stay in registers.
-            {
+            if (warp < ((c.nQ + 31u) >> 5)) {                   // warps without a unit of trials go straight to the barrier
                 philox_step ph;
 #pragma unroll
                 for (int r = 0; r < 10; ++r) {
