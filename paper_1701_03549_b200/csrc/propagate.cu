@@ -906,6 +906,7 @@ fire_init_tiles_kernel(const uint64_t* __restrict__ burnable_tiles, uint64_t* __
 }
 
 // one thread per (tile row, bitmap word column): 4 tiles in (32 B), 8 words out (one per lattice row)
+template <bool kFused>
 __global__ void __launch_bounds__(256)
 fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __restrict__ tiles, const uint32_t* __restrict__ plane_sel,
                    int planes, uint32_t* __restrict__ out_burned, int H, int Ww, int Tw, int Th, int S,
@@ -913,6 +914,7 @@ fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __rest
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool live = i < Th * Ww;                                     // no early return: the fused counts are reduced per warp
+    if (!kFused && !live) return;
     const int ty = live ? i / Ww : 0, wx = live ? i % Ww : 0;
     for (int s = blockIdx.y; s < S; s += gridDim.y) {                  // gridDim.y <= 65535 whatever the batch size
         uint32_t n_both = 0u, n_burnt = 0u;
@@ -933,11 +935,11 @@ fire_finish_kernel(const uint32_t* __restrict__ burnable, const uint64_t* __rest
                     const size_t wi = (size_t)y * Ww + wx;
                     const uint32_t bw = __ldg(burnable + wi) & ~susw;
                     out[wi] = bw;
-                    if (fit_counts) { n_burnt += __popc(bw); n_both += __popc(bw & __ldg(fit_ref + wi)); }
+                    if (kFused) { n_burnt += __popc(bw); n_both += __popc(bw & __ldg(fit_ref + wi)); }
                 }
             }
         }
-        if (fit_counts) {                                              // Eq. 2's two counts, fused (fire_set_fused_counts)
+        if (kFused) {                                                  // Eq. 2's two counts, fused (fire_set_fused_counts)
             n_both = __reduce_add_sync(0xFFFFFFFFu, n_both);
             n_burnt = __reduce_add_sync(0xFFFFFFFFu, n_burnt);
             if ((threadIdx.x & 31) == 0 && (n_both | n_burnt)) {
@@ -1532,8 +1534,9 @@ extern "C" int fire_simulate_batch(fire_landscape* L, const int32_t* ignitions, 
     if (prof) { FIRE_CUDA_TRY(L, cudaEventRecord(L->prof_ev[2 * L->prof_count + 1], st)); L->prof_count += 1; }
     {
         const size_t n = (size_t)L->Th * L->Ww;
-        fire_finish_kernel<<<dim3((unsigned)((n + 255) / 256), (unsigned)(S < 65535 ? S : 65535)), 256, 0, st>>>(L->burnable, L->tiles, L->status + S, planes, out_burned,
-                                                                                          L->H, L->Ww, L->Tw, L->Th, S, L->fit_ref, L->fit_counts);
+        const dim3 fgrid((unsigned)((n + 255) / 256), (unsigned)(S < 65535 ? S : 65535));
+        if (L->fit_counts) fire_finish_kernel<true><<<fgrid, 256, 0, st>>>(L->burnable, L->tiles, L->status + S, planes, out_burned, L->H, L->Ww, L->Tw, L->Th, S, L->fit_ref, L->fit_counts);
+        else fire_finish_kernel<false><<<fgrid, 256, 0, st>>>(L->burnable, L->tiles, L->status + S, planes, out_burned, L->H, L->Ww, L->Tw, L->Th, S, nullptr, nullptr);
         FIRE_CUDA_TRY(L, cudaGetLastError());
     }
     if (bt) fire_propagate_rescue_bt_kernel<<<kRescueCtas, 256, 0, st>>>(prm, L->rescue_planes);
