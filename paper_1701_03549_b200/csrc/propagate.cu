@@ -84,6 +84,16 @@ __device__ __forceinline__ thr_sector ldg_thr(const uint4* p)
     return v;
 }
 
+// The same sector by two loads that ptxas keeps where they are written (it sinks the one above below the warp scan and the
+// "no trials" exit to save registers, which puts the DRAM latency after the scan instead of under it).
+__device__ __forceinline__ thr_sector ldg_thr_early(const uint4* p)
+{
+    thr_sector v;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.a.x), "=r"(v.a.y), "=r"(v.a.z), "=r"(v.a.w) : "l"(p));
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0,%1,%2,%3}, [%4+16];" : "=r"(v.b.x), "=r"(v.b.y), "=r"(v.b.z), "=r"(v.b.w) : "l"(p));
+    return v;
+}
+
 __device__ __forceinline__ uint64_t ldcg_u64(const uint64_t* p) { return (uint64_t)__ldcg(reinterpret_cast<const unsigned long long*>(p)); }
 
 constexpr uint32_t kM0 = 0xD2511F53u, kM1 = 0xCD9E8D57u;       // Philox4x32 multipliers
@@ -191,7 +201,7 @@ __device__ __forceinline__ uint32_t cells_pass(const step_ctx& c, uint32_t u0, u
         const int voff = (by == 0u && ty0 > 0u) ? -(int)c.Tw : ((by == 7u && ty0 + 1u < c.Th) ? (int)c.Tw : 0);
         const uint4* const sp = c.thr4 + (size_t)(c.thr_sec + y * c.W + x) * 2;
         tc[k] = ldcg_u64(c.tiles + (c.plane_r + tidx));
-        { const thr_sector ts = ldg_thr(sp); Ta[k] = ts.a; Tb[k] = ts.b; }
+        { const thr_sector ts = (K == 1) ? ldg_thr_early(sp) : ldg_thr(sp); Ta[k] = ts.a; Tb[k] = ts.b; }
         th[k] = 0ull; tv[k] = 0ull; td[k] = 0ull;
         if (hoff) th[k] = ldcg_u64(c.tiles + (c.plane_r + tidx + hoff));
         if (voff) tv[k] = ldcg_u64(c.tiles + (c.plane_r + tidx + voff));
