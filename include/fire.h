@@ -74,7 +74,9 @@ int fire_landscape_destroy(fire_landscape* L);
 /* Contagion-threshold precompute (a2; Eq. 1).  beta f32[P][5] = (beta_0 .. beta_4).
  * For every parameter vector p, burnable cell c and direction d:
  *   T[p][c][d] = min(rint(2^32 / (1 + exp(-(b0 + b1 I_f + b2 psi + b3 omega_d + b4 sigma_d)))), 2^32 - 1)
- * in IEEE double, no FMA contraction; T = 0 on non-burnable cells.  A trial succeeds iff
+ * x in IEEE double in the written order, separate multiplies and adds (no FMA contraction); the logistic and the rounding in
+ * double precision to within ONE count of the correctly rounded value (4e-8 of the entries differ by one count from a libm
+ * evaluation, none by more: tests/test_gpu_parity.py); T = 0 on non-burnable cells.  A trial succeeds iff
  * rnd < T or T == 2^32 - 1 (R-11).  Replaces any previous table; allocates P*W*H*32 bytes. */
 int fire_params_upload(fire_landscape* L, const float* beta, int32_t P, void* stream);
 
