@@ -280,7 +280,8 @@ def test_results_do_not_depend_on_launch_geometry_or_list_capacity(request):
             (256, 4, 0, 0, 0, 2), (32, 2, 0, 0, 1, 2), (1024, 1, 0, 0, 0, 2), (512, 2, 16, 0, 0, 2),
             (256, 5, 5, 4096, 1, 2), (256, 6, 8, 8, 0, 2), (128, 4, 1, 1, 0, 2), (0, 0, 0, 0, 0, 2),
             (1024, 1, 0, 0, 0, 3), (1024, 1, 0, 0, 1, 4), (256, 2, 0, 0, 0, 4), (512, 1, 16, 0, 1, 3), (128, 4, 1, 4096, 0, 4),
-            (64, 3, 5, 4096, 1, 3), (256, 4, 8, 8, 0, 3), (32, 1, 0, 0, 0, 4), (0, 0, 0, 0, 0, 3), (0, 0, 0, 0, 1, 4)]:
+            (64, 3, 5, 4096, 1, 3), (256, 4, 8, 8, 0, 3), (32, 1, 0, 0, 0, 4), (0, 0, 0, 0, 0, 3), (0, 0, 0, 0, 1, 4),
+            (896, 1, 0, 0, 0, 3), (896, 1, 16, 0, 1, 4), (768, 1, 0, 0, 0, 2)]:
         mode = (threads, per_sm, shared, total, order, family)
         lf.fire_set_launch_geometry(L, threads, per_sm)
         lf.fire_set_list_capacity(L, shared, total)
