@@ -8,7 +8,7 @@
 //
 // Both kernels are HBM streams: a1 reads 13 B and writes 90 B per cell once per landscape; a2 writes
 // 32 B per (p, cell) -- one DRAM sector holding the 8 directions of a target cell -- and re-reads the
-// covariates of a cell once per group of FIRE_THR_PGROUP parameter vectors.
+// covariates of a cell once per CTA, i.e. once per `vectors_per_cta` parameter vectors (all of them on large lattices).
 #include "fire_internal.cuh"
 
 #include <new>
@@ -72,7 +72,7 @@ fire_covariates_kernel(const uint8_t* __restrict__ veg, const float* __restrict_
 // vectors.  The 8 thresholds of a target go through shared memory to the slots of their 8 sources, so
 // that sources whose targets all lie in the tile (30 x 6 of 32 x 8) are written as whole sectors; the
 // others are completed, 4 B at a time, by the neighbouring tiles (merged in L2).
-#define FIRE_THR_PGROUP 8
+#define FIRE_THR_PGROUP 64      // parameter vectors staged in shared memory at a time
 constexpr int kThrTX = 32, kThrTY = 8;
 
 // T = min(rint(2^32 / (1 + exp(-x))), 2^32 - 1) in double precision, written for the FP64 pipe: the kernel is bound by it (about 30
@@ -210,7 +210,7 @@ __device__ __forceinline__ float fire_thresholds_of_cell(double base, double b3,
     return fsum;
 }
 __global__ void __launch_bounds__(kThrTX * kThrTY, 4)
-fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int tiles_x,
+fire_thresholds_kernel(const float* __restrict__ beta, int P, int vectors_per_cta, int W, int H, int tiles_x,
                        const uint8_t* __restrict__ flags, const uint8_t* __restrict__ uphill,
                        const double* __restrict__ psi, const double* __restrict__ tan_slope,
                        const double* __restrict__ omega, const double* __restrict__ if_cell, uint32_t* __restrict__ thr,
@@ -222,10 +222,11 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
     __shared__ float s_mean[FIRE_THR_PGROUP];
     __shared__ uint32_t sT2[2][8][kThrTY + 2][kThrTX + 2];                // [buffer][d][source row + 1][source column + 1]
     const int tid = threadIdx.x, lx = tid & 31, ly = tid >> 5;
-    const int p0 = blockIdx.y * FIRE_THR_PGROUP;
-    const int np = min(FIRE_THR_PGROUP, P - p0);
-    if (tid < np * 5) { const float bv = beta[(size_t)p0 * 5 + tid]; sb[tid / 5][tid % 5] = (double)bv; sab[tid / 5][tid % 5] = fabsf(bv); }
-    if (tid < FIRE_THR_PGROUP) s_mean[tid] = 0.0f;
+    // this CTA's parameter vectors: [p_begin, p_end), staged through shared memory FIRE_THR_PGROUP at a time.  The covariates of the
+    // tile are loaded once per CTA (a cold DRAM round trip with nothing to overlap it), so the more vectors a CTA takes the better,
+    // as long as the grid still has a few waves (the host picks vectors_per_cta)
+    const int p_begin = blockIdx.y * vectors_per_cta;
+    const int p_end = min(P, p_begin + vectors_per_cta);
     if (tid < 64) s_exp2[tid] = kExp2Table[tid];
     const int x0 = (int)(blockIdx.x % tiles_x) * kThrTX, y0 = (int)(blockIdx.x / tiles_x) * kThrTY;
     const int x = x0 + lx, y = y0 + ly;
@@ -279,6 +280,11 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
         }
     }
     const int hx1 = hx + 1, hy1 = hy + 1;
+    for (int p0 = p_begin; p0 < p_end; p0 += FIRE_THR_PGROUP) {
+    const int np = min(FIRE_THR_PGROUP, p_end - p0);
+    __syncthreads();                                                      // the previous chunk's last reads of sb, s_mean and sT2
+    for (int i = tid; i < np * 5; i += kThrTX * kThrTY) { const float bv = beta[(size_t)p0 * 5 + i]; sb[i / 5][i % 5] = (double)bv; sab[i / 5][i % 5] = fabsf(bv); }
+    if (tid < FIRE_THR_PGROUP) s_mean[tid] = 0.0f;
     __syncthreads();
     for (int q = 0; q < np; ++q) {
         const double b0 = sb[q][0], b1 = sb[q][1], b2 = sb[q][2], b3 = sb[q][3], b4 = sb[q][4];
@@ -320,6 +326,7 @@ fire_thresholds_kernel(const float* __restrict__ beta, int P, int W, int H, int 
     }
     __syncthreads();
     if (tid < np) atomicAdd(param_mean + p0 + tid, s_mean[tid]);
+    }
 }
 
 // Test hook: the table of one parameter vector in TARGET-indexed form out[c][d] = T(target c, direction d).
@@ -508,8 +515,14 @@ extern "C" int fire_params_upload(fire_landscape* L, const float* beta, int32_t 
     }
     FIRE_CUDA_TRY(L, cudaMemsetAsync(L->param_mean, 0, (size_t)P * sizeof(float), (cudaStream_t)stream));
     const int tiles_x = (L->W + kThrTX - 1) / kThrTX, tiles_y = (L->H + kThrTY - 1) / kThrTY;
-    dim3 grid((unsigned)(tiles_x * tiles_y), (unsigned)((P + FIRE_THR_PGROUP - 1) / FIRE_THR_PGROUP));
-    fire_thresholds_kernel<<<grid, kThrTX * kThrTY, 0, (cudaStream_t)stream>>>(L->beta_dev, P, L->W, L->H, tiles_x, L->flags,
+    // vectors per CTA: as many as leave about eight waves of CTAs (4 resident per SM), at least 8 (one group of the old scheme)
+    const long long tiles = (long long)tiles_x * tiles_y;
+    long long gy = (8ll * 4 * L->num_sms + tiles - 1) / tiles;
+    if (gy < 1) gy = 1;
+    if (gy > (P + 7) / 8) gy = (P + 7) / 8;
+    const int vectors_per_cta = (int)((P + gy - 1) / gy);
+    dim3 grid((unsigned)tiles, (unsigned)((P + vectors_per_cta - 1) / vectors_per_cta));
+    fire_thresholds_kernel<<<grid, kThrTX * kThrTY, 0, (cudaStream_t)stream>>>(L->beta_dev, P, vectors_per_cta, L->W, L->H, tiles_x, L->flags,
                                                                                 L->uphill, L->psi, L->tan_slope, L->omega, L->if_cell, L->thr, L->param_mean);
     L->launches += 1;
     FIRE_CUDA_TRY(L, cudaGetLastError());
