@@ -50,8 +50,8 @@ UNIT = "trials/s"
 # ncu --set full capture of the propagation kernel on the workload below: dram__bytes_read.sum + dram__bytes_write.sum per
 # launch, with the commit the captured kernel was built from (profiles/README.md names the file and the command).  Refresh
 # the number together with every change of the propagation kernel; None until a capture exists for that config.
-NCU_TRAFFIC_BYTES = {3: 17894972000 + 206632000}      # profiles/r2_propagate_ncu.md: capture of commit bccb42e
-NCU_TRAFFIC_SOURCE = {3: "profiles/r2_propagate_ncu.md (ncu --set full; two-phase kernel as of commit bccb42e)"}
+NCU_TRAFFIC_BYTES = {3: 17864354000 + 212908000}      # profiles/r2_propagate_ncu.md: capture of commit 1aef2ce
+NCU_TRAFFIC_SOURCE = {3: "profiles/r2_propagate_ncu.md (ncu --set full; two-phase kernel as of commit 1aef2ce)"}
 
 
 def log(*a):
