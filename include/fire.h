@@ -55,6 +55,7 @@ extern "C" {
 #define FIRE_ENOMEM  (-2)   /* device allocation failed */
 #define FIRE_ESTATE  (-3)   /* simulate before fire_params_upload, p out of range in download */
 #define FIRE_ECUDA   (-4)   /* a CUDA call failed (sticky), or no CUDA device */
+#define FIRE_ELIMIT  (-5)   /* fire_fitness_static: S beyond FIRE_FITNESS_STATIC_MAX_SIMS */
 
 #define FIRE_METRIC_DELTA    0   /* Eq. 2: (#(A u A*) - #(A n A*)) / #A, 0 = perfect overlap */
 #define FIRE_METRIC_JACCARD  1   /* #(A n A*) / #(A u A*) */
@@ -136,6 +137,19 @@ int fire_set_burn_time(fire_landscape* L, const uint8_t* burn_time_host, int32_t
  * N = #A; one IEEE divide (N = 0 gives inf/NaN, not an error).  out_ref_area u32[1] or NULL = N. */
 int fire_fitness(fire_landscape* L, const uint32_t* reference, const uint32_t* burned, int32_t S,
                  int32_t metric, float* out_score, uint32_t* out_counts, uint32_t* out_ref_area, void* stream);
+
+/* Fitness reduction that ALLOCATES NOTHING: for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it).  Same result as fire_fitness (Eq. 2; scores bit for bit) without a handle: reference
+ * u32[H][ceil(W/32)], burned u32[S][H][ceil(W/32)], out_score f32[S], out_ref_area u32[1] or NULL, all DEVICE pointers on the
+ * CURRENT device; the work is enqueued on `stream`.  The per-simulation counts (I, N*) and #A live in a static device array inside
+ * the library, sized for S <= FIRE_FITNESS_STATIC_MAX_SIMS (128.25 KiB, held by every GPU that loads the library until the process
+ * exits); a larger S returns FIRE_ELIMIT before anything is enqueued (split the batch: the score of a simulation does not depend
+ * on the others).  The call makes no cudaMalloc / cudaFree and calls no allocating library routine.  EVERY call on a device
+ * shares that one array (it is cleared at the start of each call): calls that overlap on the GPU -- two streams, or two host
+ * threads -- race on it and give wrong scores; calls on one stream, or otherwise ordered, are safe. */
+#define FIRE_FITNESS_STATIC_MAX_SIMS 16384
+int fire_fitness_static(const uint32_t* reference, const uint32_t* burned, int32_t W, int32_t H, int32_t S,
+                        int32_t metric, float* out_score, uint32_t* out_ref_area, void* stream);
 
 /* Per-candidate statistics over R replicates (a8; BASELINE config 4).
  * counts u32[G*R][2] = (I, N*), candidate-major; x = ref_area + N* - 2I.

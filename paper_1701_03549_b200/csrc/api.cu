@@ -113,6 +113,7 @@ extern "C" const char* fire_error_string(int code)
         case FIRE_ENOMEM: return "device allocation failed";
         case FIRE_ESTATE: return "call out of order (no thresholds uploaded, or parameter index out of range)";
         case FIRE_ECUDA:  return "CUDA error or no CUDA device";
+        case FIRE_ELIMIT: return "size beyond the limit of the static scratch array (FIRE_FITNESS_STATIC_MAX_SIMS)";
         default:          return "unknown error code";
     }
 }

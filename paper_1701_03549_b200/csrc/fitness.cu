@@ -9,6 +9,14 @@
 // the reference map (one plane) stays in L2.
 #include "fire_internal.cuh"
 
+#include <atomic>
+
+// Scratch of fire_fitness_static, the entry point that allocates nothing (fire.h): counts (I, N*) of up to
+// FIRE_FITNESS_STATIC_MAX_SIMS simulations, then #A of the reference map in the first word of a 256 B tail.  Every GPU that
+// loads the library holds these 128.25 KiB until the process exits.  In host code this name is a host-side stand-in, not a
+// device address: the address a kernel can use comes from cudaGetSymbolAddress (fire_static_scratch below).
+static __device__ __align__(256) uint32_t g_fitness_static_scratch[2 * FIRE_FITNESS_STATIC_MAX_SIMS + 64];
+
 namespace {
 
 __device__ __forceinline__ uint32_t warp_sum(uint32_t v)
@@ -230,6 +238,60 @@ extern "C" int fire_fitness_group_stats(const uint32_t* counts, uint32_t ref_are
     const size_t threads = (size_t)G * 32;
     fire_group_stats_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, (cudaStream_t)stream>>>(
         counts, ref_area, G, R, (unsigned long long*)out_sums, out_mean_var);
+    if (cudaGetLastError() != cudaSuccess) return FIRE_ECUDA;
+    return FIRE_OK;
+}
+
+// Device address of g_fitness_static_scratch on the CURRENT device, looked up once per device (with that device current) and
+// kept; cudaGetSymbolAddress allocates nothing (the array is part of the loaded module) and is idempotent, so two threads
+// that race here store the same value.
+static int fire_static_scratch(uint32_t** out)
+{
+    constexpr int kMaxDevices = 64;
+    static std::atomic<uint32_t*> table[kMaxDevices];
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return FIRE_ECUDA;
+    uint32_t* p = table[dev].load(std::memory_order_acquire);
+    if (p == nullptr) {
+        void* sym = nullptr;
+        if (cudaGetSymbolAddress(&sym, g_fitness_static_scratch) != cudaSuccess || sym == nullptr) {
+            (void)cudaGetLastError();
+            return FIRE_ECUDA;
+        }
+        p = static_cast<uint32_t*>(sym);
+        table[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return FIRE_OK;
+}
+
+// Eq. 2 without a handle and without any allocation (fire.h): the kernels of fire_fitness on the static scratch array.
+extern "C" int fire_fitness_static(const uint32_t* reference, const uint32_t* burned, int32_t W, int32_t H, int32_t S,
+                                   int32_t metric, float* out_score, uint32_t* out_ref_area, void* stream)
+{
+    if (!reference || !burned || !out_score || S < 1 || W < 1 || H < 1 || W > 8192 || H > 8192) return FIRE_EINVAL;
+    if (metric != FIRE_METRIC_DELTA && metric != FIRE_METRIC_JACCARD) return FIRE_EINVAL;
+    if (S > FIRE_FITNESS_STATIC_MAX_SIMS) return FIRE_ELIMIT;
+    uint32_t* scratch = nullptr;
+    const int rc = fire_static_scratch(&scratch);
+    if (rc != FIRE_OK) return rc;
+    uint32_t* const counts = scratch;
+    uint32_t* const ref_area = scratch + 2 * FIRE_FITNESS_STATIC_MAX_SIMS;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t nw = (size_t)H * (size_t)((W + 31) / 32);
+    uint32_t words_per_cta = 16384;
+    if ((size_t)words_per_cta > nw) words_per_cta = (uint32_t)((nw + 3) & ~(size_t)3);
+    const unsigned chunks = (unsigned)((nw + words_per_cta - 1) / words_per_cta);
+    // the array keeps the last call's contents: the sums of this call start at zero
+    if (cudaMemsetAsync(counts, 0, (size_t)S * 8, st) != cudaSuccess) return FIRE_ECUDA;
+    if (cudaMemsetAsync(ref_area, 0, sizeof(uint32_t), st) != cudaSuccess) return FIRE_ECUDA;
+    {
+        unsigned ctas = (unsigned)((nw + 256 * 4 - 1) / (256 * 4));
+        if (ctas > 256) ctas = 256;
+        fire_reference_area_kernel<<<ctas, 256, 0, st>>>(reference, nw, ref_area);
+    }
+    fire_fitness_counts_kernel<<<dim3(chunks, (unsigned)S), 256, 0, st>>>(reference, burned, nw, words_per_cta, counts);   // S <= 16,384 < 65,535
+    fire_fitness_score_kernel<<<(S + 255) / 256, 256, 0, st>>>(counts, ref_area, S, metric, out_score, out_ref_area);
     if (cudaGetLastError() != cudaSuccess) return FIRE_ECUDA;
     return FIRE_OK;
 }

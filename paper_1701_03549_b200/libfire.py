@@ -14,13 +14,14 @@ import torch
 _PKG = Path(__file__).resolve().parent
 LIB_PATH = _PKG / "libfire_sm100a.so"
 
-FIRE_OK, FIRE_EINVAL, FIRE_ENOMEM, FIRE_ESTATE, FIRE_ECUDA = 0, -1, -2, -3, -4
+FIRE_OK, FIRE_EINVAL, FIRE_ENOMEM, FIRE_ESTATE, FIRE_ECUDA, FIRE_ELIMIT = 0, -1, -2, -3, -4, -5
+FIRE_FITNESS_STATIC_MAX_SIMS = 16384
 FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD = 0, 1
 
 # every symbol include/fire.h declares (tests check the library exports exactly these)
 SYMBOLS = [
     "fire_landscape_create", "fire_landscape_destroy", "fire_params_upload", "fire_simulate_batch",
-    "fire_fitness", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
+    "fire_fitness", "fire_fitness_static", "fire_fitness_group_stats", "fire_thresholds_download", "fire_generation_host",
     "fire_launch_count", "fire_set_launch_geometry", "fire_set_list_capacity", "fire_set_schedule", "fire_set_kernel", "fire_set_burn_time", "fire_set_time_output", "fire_set_fused_counts", "fire_landscape_set_elevation", "fire_landscape_set_class_indicator", "fire_burn_count", "fire_error_string",
     "fire_set_profiling", "fire_profile_read",
 ]
@@ -50,6 +51,7 @@ def load() -> C.CDLL:
     lib.fire_params_upload.argtypes = [_vp, _vp, C.c_int32, _vp]
     lib.fire_simulate_batch.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_uint32, _vp, _vp, _vp, _vp]
     lib.fire_fitness.argtypes = [_vp, _vp, _vp, C.c_int32, C.c_int32, _vp, _vp, _vp, _vp]
+    lib.fire_fitness_static.argtypes = [_vp, _vp, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp, _vp, _vp]
     lib.fire_fitness_group_stats.argtypes = [_vp, C.c_uint32, C.c_int32, C.c_int32, _vp, _vp, _vp]
     lib.fire_thresholds_download.argtypes = [_vp, C.c_int32, _vp, _vp]
     lib.fire_generation_host.argtypes = [_vp, _vp, C.c_int32, _vp, _vp, _vp, _vp, C.c_int32, C.c_uint32, _vp,
@@ -192,6 +194,20 @@ def fire_fitness(L: Landscape, reference: torch.Tensor, burned: torch.Tensor, me
         _dev(burned, torch.int32, "burned", (S, L.H, L.Ww)), S, int(metric),
         _dev(out_score, torch.float32, "out_score", (S,)), _dev(out_counts, torch.int32, "out_counts", (S, 2)),
         _dev(out_ref_area, torch.int32, "out_ref_area", (1,)), _stream(stream)), "fire_fitness")
+
+
+def fire_fitness_static(reference: torch.Tensor, burned: torch.Tensor, W: int, metric: int, out_score: torch.Tensor,
+                        out_ref_area: torch.Tensor | None = None, stream=None) -> None:
+    """fire_fitness without a handle and without any device allocation (scratch in a static device array of the library):
+    reference i32[H][Ww], burned i32[S][H][Ww] -> out_score f32[S], out_ref_area i32[1]; S <= FIRE_FITNESS_STATIC_MAX_SIMS."""
+    S, H, Ww = (int(v) for v in burned.shape)
+    if Ww != (int(W) + 31) // 32:
+        raise ValueError("burned: last dimension must be ceil(W / 32)")
+    with torch.cuda.device(burned.device):
+        _check(load().fire_fitness_static(
+            _dev(reference, torch.int32, "reference", (H, Ww)), _dev(burned, torch.int32, "burned", (S, H, Ww)),
+            int(W), H, S, int(metric), _dev(out_score, torch.float32, "out_score", (S,)),
+            _dev(out_ref_area, torch.int32, "out_ref_area", (1,)), _stream(stream)), "fire_fitness_static")
 
 
 def fire_fitness_group_stats(counts: torch.Tensor, ref_area: int, G: int, R: int, out_sums: torch.Tensor,

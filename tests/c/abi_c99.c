@@ -25,8 +25,9 @@ typedef int (*elev_fn)(fire_landscape*, const float*, void*);
 typedef int (*hazard_fn)(fire_landscape*, const uint32_t*, int32_t, uint32_t*, void*);
 typedef int (*timeout_fn)(fire_landscape*, int32_t*);
 typedef int (*fused_fn)(fire_landscape*, const uint32_t*, uint32_t*);
+typedef int (*static_fn)(const uint32_t*, const uint32_t*, int32_t, int32_t, int32_t, int32_t, float*, uint32_t*, void*);
 typedef int (*classif_fn)(fire_landscape*, const float*, int32_t, void*);
-any_fn fire_abi_table[22];
+any_fn fire_abi_table[23];
 
 void fire_abi_fill(void)
 {
@@ -44,6 +45,8 @@ void fire_abi_fill(void)
     timeout_fn f19 = fire_set_time_output;
     classif_fn f20 = fire_landscape_set_class_indicator;
     fused_fn f21 = fire_set_fused_counts;
+    static_fn f22 = fire_fitness_static;
+    fire_abi_table[22] = (any_fn)f22;
     fire_abi_table[21] = (any_fn)f21;
     fire_abi_table[20] = (any_fn)f20;
     fire_abi_table[19] = (any_fn)f19;
@@ -56,6 +59,7 @@ void fire_abi_fill(void)
     fire_abi_table[10] = (any_fn)f10; fire_abi_table[11] = (any_fn)f11;
     fire_abi_table[12] = (any_fn)f12; fire_abi_table[13] = (any_fn)f13;
     fire_abi_table[14] = (any_fn)f14; fire_abi_table[15] = (any_fn)f15;
-    { int codes[5] = { FIRE_OK, FIRE_EINVAL, FIRE_ENOMEM, FIRE_ESTATE, FIRE_ECUDA }; (void)codes; }
+    { int codes[6] = { FIRE_OK, FIRE_EINVAL, FIRE_ENOMEM, FIRE_ESTATE, FIRE_ECUDA, FIRE_ELIMIT }; (void)codes; }
+    { int limits[1] = { FIRE_FITNESS_STATIC_MAX_SIMS }; (void)limits; }
     { int metrics[2] = { FIRE_METRIC_DELTA, FIRE_METRIC_JACCARD }; (void)metrics; }
 }
